@@ -1,0 +1,136 @@
+/* include/lbm.h -- C ABI of liblbm_b200.so: the fused LBM stream-collide time step with decoupled
+ * arithmetic (FP32) and storage (FP32 / 16-bit) precision, for one NVIDIA B200 (sm_100a).
+ *
+ * The method is the one of Lehmann et al., arXiv 2112.08926 ("PAPER.md" below = the paper text,
+ * cited as PAPER.md:<line>); every reading of a silent / garbled passage is listed in DESIGN.md
+ * section 3 ("R<n>").  Nothing here is torch-typed: plain pointers and sizes.  Each pointer argument
+ * says whether it is a HOST or a DEVICE pointer.
+ *
+ * Conventions
+ *   - every function returns an int status: LBM_OK (0) or a negative LBM_E_* code; no C++ exception
+ *     crosses the boundary; lbm_last_error() gives a thread-local human-readable message.
+ *   - cell index n = x + nx*(y + ny*z); N = nx*ny*nz.
+ *   - DDF buffers are structure-of-arrays [q][N], element = float (LBM_FP32) or
+ *     uint16 (all other formats); the library keeps two of them (A-B / one-step pull).
+ *     The stored quantity is the SHIFTED DDF f_i - w_i.
+ *   - rho is float [N]; u is float [3][N] (ux | uy | uz).
+ *   - flags are 1 byte per cell; bit LBM_FLAG_WALL (TYPE_W) marks a halfway
+ *     bounce-back wall cell.  The u entries of a wall cell are the wall velocity (moving wall, R9).
+ *   - all faces are periodic; solid boundaries exist only as wall cells.
+ *   - a handle is bound to the CUDA device that was current at lbm_create and to one stream; calls on
+ *     one handle must not race.  lbm_step is asynchronous on that stream; everything that returns data
+ *     to the host synchronises the stream.
+ *   - there is NO CPU fallback: without a usable CUDA device lbm_create fails with LBM_E_CUDA.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbm lbm_t; /* opaque, owned by the library, freed by lbm_destroy */
+
+/* velocity sets (R1: D3Q19 numbering from PAPER.md:955-959, 1029-1031; D2Q9 needs nz == 1) */
+enum { LBM_D2Q9 = 9, LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
+/* collision operators.  BGK = eq (28).  TRT is named but never
+ * defined by the paper: lbm_create answers LBM_E_UNSUPPORTED for LBM_TRT (R13). */
+enum { LBM_BGK = 0, LBM_TRT = 1 };
+/* DDF storage formats (Table 2, 152-178, 201-219; Listing 1) */
+enum {
+    LBM_FP32 = 0,   /* IEEE binary32, identity load/store                        */
+    LBM_FP16S = 1,  /* IEEE binary16 of x*2^15, round-to-nearest-even   */
+    LBM_FP16C = 2,  /* custom 1-4-11, bias 15, no Inf/NaN, saturating   */
+    LBM_P16_0S = 3, /* posit<16,0>, sign-magnitude, scaled by 2^7      */
+    LBM_P16_1S = 4, /* posit<16,1>, sign-magnitude, scaled by 2^7  */
+    LBM_P16_2C = 5, /* one-sided regime, 2 exponent bits, unscaled */
+    LBM_FP16 = 6    /* plain IEEE binary16 (Table 2 row 139)                          */
+};
+enum { LBM_FLAG_WALL = 0x01 };
+enum {
+    LBM_OK = 0,
+    LBM_E_INVAL = -1,       /* bad argument                                   */
+    LBM_E_UNSUPPORTED = -2, /* valid request the library does not implement   */
+    LBM_E_NOMEM = -3,       /* device or host allocation failed               */
+    LBM_E_CUDA = -4,        /* CUDA runtime error (message in lbm_last_error) */
+    LBM_E_STATE = -5        /* call sequence violated                         */
+};
+
+/* Create a simulation.  nx, ny, nz >= 1 (nz == 1 for LBM_D2Q9); tau > 0.5 (omega = 1/tau,
+ * PAPER.md:707); force: HOST pointer to 3 floats (uniform body force, Guo forcing R10) or NULL.
+ * Allocates the flags (all fluid) but no DDF memory: that happens at the first lbm_bind / lbm_init.
+ * On success *out is the new handle. */
+int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, int ddf_format, float tau,
+               const float *force);
+
+/* Optional: run on caller-owned device memory and/or a caller-owned stream (e.g. torch tensors and
+ * torch's current stream).  ddf_a, ddf_b: DEVICE pointers, each at least lbm_ddf_buffer_bytes() bytes,
+ * 16-byte aligned, must outlive the handle; both NULL = library allocates.  cuda_stream: a cudaStream_t
+ * cast to void* (NULL = the legacy default stream).  Must be called before lbm_init. */
+int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream);
+
+/* Tuning knob: cells per thread of the stream_collide kernel, v in {0 = automatic, 1, 2, 4}; nx must be
+ * a multiple of v.  The result of a run does not depend on it (tests check that bit for bit). */
+int lbm_set_cells_per_thread(lbm_t *h, int v);
+
+/* Set the cell flags.  flags: HOST pointer, N bytes, copied.  Only LBM_FLAG_WALL may be set
+ * (else LBM_E_INVAL).  Must precede lbm_init (LBM_E_STATE otherwise).  Synchronises the stream. */
+int lbm_set_flags(lbm_t *h, const unsigned char *flags);
+
+/* Initialise every cell, walls included, in both DDF buffers with the shifted equilibrium
+ * f_i^eq(rho[n], u[n]) of eq (3) (R11) and reset the step counter.
+ * rho: N floats, u: 3N floats (SoA).  lbm_init takes HOST pointers (copied, synchronous);
+ * lbm_init_device takes DEVICE pointers read asynchronously on the handle's stream. */
+int lbm_init(lbm_t *h, const float *rho, const float *u);
+int lbm_init_device(lbm_t *h, const float *rho_dev, const float *u_dev);
+
+/* Advance n >= 0 time steps: n launches of the fused stream-collide kernel (Listing 2,
+ * PAPER.md:1014-1042; eqs (24)-(28)), alternating the two buffers.
+ * Asynchronous on the handle's stream. */
+int lbm_step(lbm_t *h, int n);
+
+/* Density and velocity "after the steps done so far" = local moments of the current buffer (R12;
+ * PAPER.md:428, 951-968); wall cells return the values given to lbm_init.  Either pointer may be NULL.
+ * lbm_read_rho_u: HOST pointers, synchronises.  lbm_read_rho_u_device: DEVICE pointers, asynchronous. */
+int lbm_read_rho_u(lbm_t *h, float *rho, float *u);
+int lbm_read_rho_u_device(lbm_t *h, float *rho_dev, float *u_dev);
+
+/* Copy direction i (0 <= i < q) of the current DDF buffer, as stored (N elements of 2 or 4 bytes),
+ * to a HOST pointer.  Synchronises.  For bit-level parity tests. */
+int lbm_read_ddf(lbm_t *h, int i, void *out);
+
+/* Block until all work queued on the handle's stream has finished. */
+int lbm_sync(lbm_t *h);
+/* Steps done since the last lbm_init. */
+long long lbm_steps_done(const lbm_t *h);
+/* Free the handle and everything the library allocated for it (not caller-bound memory). */
+int lbm_destroy(lbm_t *h);
+
+/* Message of the last failing call on this thread ("" if none). */
+const char *lbm_last_error(void);
+
+/* ---- storage-format codecs, exposed for bit-level parity tests and micro-benchmarks ------------
+ * store(): FP32 -> 16-bit code; load(): code -> FP32.  ddf_format in
+ * LBM_FP16S..LBM_FP16.  *_device variants take DEVICE pointers and run asynchronously on `cuda_stream`
+ * (cudaStream_t as void*, NULL = default stream); the plain variants take HOST pointers. */
+int lbm_codec_encode(int ddf_format, const float *x, unsigned short *codes, long long count);
+int lbm_codec_decode(int ddf_format, const unsigned short *codes, float *x, long long count);
+int lbm_codec_encode_device(int ddf_format, const float *x_dev, unsigned short *codes_dev, long long count,
+                            void *cuda_stream);
+int lbm_codec_decode_device(int ddf_format, const unsigned short *codes_dev, float *x_dev, long long count,
+                            void *cuda_stream);
+
+/* ---- sizes -------------------------------------------------------------------------------------*/
+/* bytes of ONE DDF buffer: q * N * sizeof(element), rounded up to a multiple of 256 */
+long long lbm_ddf_buffer_bytes(int nx, int ny, int nz, int velset, int ddf_format);
+/* algorithmic DRAM traffic of one cell update: 2*q*sizeof(element) + 1 flag byte */
+long long lbm_bytes_per_cell(int velset, int ddf_format);
+/* name of the stream_collide kernel variant the handle dispatches to (for profiles), "" before init */
+const char *lbm_kernel_name(const lbm_t *h);
+/* number of kernels this library has launched in this process (all handles), for bench accounting */
+long long lbm_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

@@ -1,0 +1,393 @@
+// lbm_api.cu -- the C ABI of include/lbm.h.  Host logic only: argument checks, device memory, the
+// A/B buffer swap and kernel dispatch.  Every step of the path itself runs in the CUDA kernels of
+// lbm_kernels.cuh; there is no CPU implementation of any of it in this library.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/lbm.h"
+#include "lbm_internal.h"
+
+namespace lbmk {
+long long launches();
+}
+
+using lbmk::Params;
+using lbmk::UnitOps;
+
+struct lbm {
+    int nx, ny, nz, q, fmt, collision;
+    long long N;
+    float tau, omega;
+    float force[3];
+    bool has_force;
+    int device;
+    cudaStream_t stream;
+    unsigned char *flags;      // device, N bytes, bit 0 = wall, bit 7 = FLAG_NEAR
+    bool has_walls;
+    void *ddf[2];              // device, SoA [q][N]
+    bool owns_ddf, bound;
+    int cur;                   // index of the buffer holding the current state
+    float *rho0, *u0;          // device copies of the init fields, kept only when the box has walls
+    long long steps;
+    bool inited;
+    int V;                     // cells per thread of the stream_collide variant in use
+    int V_request;             // 0 = automatic
+    const UnitOps *ops;
+};
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg) {
+    g_err = msg;
+    return code;
+}
+
+#define LBM_CUDA_TRY(expr)                                                                              \
+    do {                                                                                                \
+        cudaError_t e_ = (expr);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            (void)cudaGetLastError();                                                                   \
+            return fail(e_ == cudaErrorMemoryAllocation ? LBM_E_NOMEM : LBM_E_CUDA,                     \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                            \
+        }                                                                                               \
+    } while (0)
+
+int elem_size(int fmt) { return fmt == LBM_FP32 ? 4 : 2; }
+bool valid_velset(int v) { return v == LBM_D2Q9 || v == LBM_D3Q19 || v == LBM_D3Q27; }
+bool valid_format(int f) { return f >= LBM_FP32 && f <= LBM_FP16; }
+
+Params make_params(const lbm *h) {
+    Params p;
+    p.nx = h->nx; p.ny = h->ny; p.nz = h->nz;
+    p.N = h->N;
+    p.omega = h->omega;
+    p.one_m_omega = 1.0f - h->omega;
+    p.omega_minus = 0.0f;
+    p.one_m_omega_minus = 0.0f;
+    p.fx = h->force[0]; p.fy = h->force[1]; p.fz = h->force[2];
+    p.flags = h->flags;
+    p.rho0 = h->rho0;
+    p.u0 = h->u0;
+    return p;
+}
+
+int enter(lbm *h) {
+    if (!h) return fail(LBM_E_INVAL, "null handle");
+    LBM_CUDA_TRY(cudaSetDevice(h->device));
+    return LBM_OK;
+}
+
+int ensure_ddf(lbm *h) {
+    if (h->ddf[0]) return LBM_OK;
+    const long long bytes = lbm_ddf_buffer_bytes(h->nx, h->ny, h->nz, h->q, h->fmt);
+    for (int b = 0; b < 2; ++b) {
+        cudaError_t e = cudaMalloc(&h->ddf[b], (size_t)bytes);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            if (b == 1) { cudaFree(h->ddf[0]); }
+            h->ddf[0] = h->ddf[1] = nullptr;
+            return fail(LBM_E_NOMEM, std::string("cudaMalloc of a DDF buffer: ") + cudaGetErrorString(e));
+        }
+    }
+    h->owns_ddf = true;
+    return LBM_OK;
+}
+
+// cells per thread: the widest of {4, 2, 1} that divides nx (vector loads must not straddle a row);
+// the per-format default comes from the bandwidth sweep recorded in DESIGN.md section 5
+int pick_cells_per_thread(const lbm *h) {
+    int want = h->V_request;
+    if (want == 0) {
+        const char *env = getenv("LBM_CELLS_PER_THREAD");
+        if (env && *env) want = atoi(env);
+    }
+    if (want == 0) want = 2;
+    if (want != 1 && want != 2 && want != 4) want = 1;
+    while (want > 1 && h->nx % want != 0) want >>= 1;
+    return want;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *lbm_last_error(void) { return g_err.c_str(); }
+
+long long lbm_launch_count(void) { return lbmk::launches(); }
+
+long long lbm_ddf_buffer_bytes(int nx, int ny, int nz, int velset, int ddf_format) {
+    if (nx < 1 || ny < 1 || nz < 1 || !valid_velset(velset) || !valid_format(ddf_format)) return -1;
+    const long long bytes = (long long)nx * ny * nz * velset * elem_size(ddf_format);
+    return (bytes + 255) / 256 * 256;
+}
+
+long long lbm_bytes_per_cell(int velset, int ddf_format) {
+    if (!valid_velset(velset) || !valid_format(ddf_format)) return -1;
+    return 2LL * velset * elem_size(ddf_format) + 1;
+}
+
+int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, int ddf_format, float tau,
+               const float *force) {
+    if (!out) return fail(LBM_E_INVAL, "lbm_create: out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_E_INVAL, "lbm_create: nx, ny, nz must be >= 1");
+    if (ny > 65535 || nz > 65535) return fail(LBM_E_INVAL, "lbm_create: ny and nz must be <= 65535 (CUDA grid limit)");
+    if (!valid_velset(velset)) return fail(LBM_E_INVAL, "lbm_create: velset must be 9, 19 or 27");
+    if (velset == LBM_D2Q9 && nz != 1) return fail(LBM_E_INVAL, "lbm_create: D2Q9 needs nz == 1");
+    if (!valid_format(ddf_format)) return fail(LBM_E_INVAL, "lbm_create: unknown ddf_format");
+    if (collision == LBM_TRT) return fail(LBM_E_UNSUPPORTED, "lbm_create: TRT is named but not defined by the paper (PAPER.md:43)");
+    if (collision != LBM_BGK) return fail(LBM_E_INVAL, "lbm_create: unknown collision operator");
+    if (!(tau > 0.5f)) return fail(LBM_E_INVAL, "lbm_create: tau must be > 0.5 (PAPER.md:79)");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        (void)cudaGetLastError();
+        return fail(LBM_E_CUDA, "lbm_create: no CUDA device (this library has no CPU fallback)");
+    }
+    lbm *h = new (std::nothrow) lbm();
+    if (!h) return fail(LBM_E_NOMEM, "lbm_create: out of host memory");
+    std::memset(h, 0, sizeof *h);
+    h->nx = nx; h->ny = ny; h->nz = nz; h->q = velset; h->fmt = ddf_format; h->collision = collision;
+    h->N = (long long)nx * ny * nz;
+    h->tau = tau;
+    h->omega = 1.0f / tau;
+    for (int a = 0; a < 3; ++a) {
+        h->force[a] = force ? force[a] : 0.0f;
+        if (h->force[a] != 0.0f) h->has_force = true;
+    }
+    h->ops = lbmk::unit_ops(velset, ddf_format);
+    if (!h->ops) { delete h; return fail(LBM_E_UNSUPPORTED, "lbm_create: no kernel unit for this velset/format"); }
+    cudaError_t e = cudaGetDevice(&h->device);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->flags, (size_t)h->N);
+    if (e == cudaSuccess) e = cudaMemset(h->flags, 0, (size_t)h->N);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (h->flags) cudaFree(h->flags);
+        delete h;
+        return fail(e == cudaErrorMemoryAllocation ? LBM_E_NOMEM : LBM_E_CUDA, std::string("lbm_create: ") + cudaGetErrorString(e));
+    }
+    *out = h;
+    return LBM_OK;
+}
+
+int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream) {
+    if (int rc = enter(h)) return rc;
+    if (h->inited) return fail(LBM_E_STATE, "lbm_bind: must be called before lbm_init");
+    if ((ddf_a == nullptr) != (ddf_b == nullptr)) return fail(LBM_E_INVAL, "lbm_bind: bind both DDF buffers or neither");
+    if (ddf_a) {
+        if (((size_t)ddf_a | (size_t)ddf_b) & 15) return fail(LBM_E_INVAL, "lbm_bind: DDF buffers must be 16-byte aligned");
+        if (ddf_a == ddf_b) return fail(LBM_E_INVAL, "lbm_bind: the two DDF buffers must be distinct");
+        if (h->owns_ddf) { cudaFree(h->ddf[0]); cudaFree(h->ddf[1]); h->owns_ddf = false; }
+        h->ddf[0] = ddf_a;
+        h->ddf[1] = ddf_b;
+    }
+    h->stream = (cudaStream_t)cuda_stream;
+    h->bound = true;
+    return LBM_OK;
+}
+
+int lbm_set_cells_per_thread(lbm_t *h, int v) {
+    if (int rc = enter(h)) return rc;
+    if (v != 0 && v != 1 && v != 2 && v != 4) return fail(LBM_E_INVAL, "lbm_set_cells_per_thread: 0 (auto), 1, 2 or 4");
+    if (v > 1 && h->nx % v != 0) return fail(LBM_E_INVAL, "lbm_set_cells_per_thread: nx must be a multiple of v");
+    h->V_request = v;
+    h->V = pick_cells_per_thread(h);
+    return LBM_OK;
+}
+
+int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
+    if (int rc = enter(h)) return rc;
+    if (!flags) return fail(LBM_E_INVAL, "lbm_set_flags: flags is NULL");
+    if (h->inited) return fail(LBM_E_STATE, "lbm_set_flags: must be called before lbm_init");
+    bool walls = false;
+    for (long long n = 0; n < h->N; ++n) {
+        if (flags[n] & ~LBM_FLAG_WALL) return fail(LBM_E_INVAL, "lbm_set_flags: unknown flag bit set");
+        walls |= flags[n] != 0;
+    }
+    h->has_walls = walls;
+    if (!walls) {
+        LBM_CUDA_TRY(cudaMemsetAsync(h->flags, 0, (size_t)h->N, h->stream));
+        LBM_CUDA_TRY(cudaStreamSynchronize(h->stream));
+        return LBM_OK;
+    }
+    unsigned char *tmp = nullptr;
+    LBM_CUDA_TRY(cudaMalloc((void **)&tmp, (size_t)h->N));
+    cudaError_t e = cudaMemcpyAsync(tmp, flags, (size_t)h->N, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = lbmk::launch_mark_near(h->q, tmp, h->flags, h->nx, h->ny, h->nz, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(tmp);
+    LBM_CUDA_TRY(e);
+    return LBM_OK;
+}
+
+static int init_from_device(lbm *h, const float *rho_dev, const float *u_dev) {
+    if (int rc = ensure_ddf(h)) return rc;
+    const float *r = rho_dev, *u = u_dev;
+    if (h->has_walls) {                          // wall velocity (R9) and wall read-out (R12) need the init fields later
+        if (!h->rho0) LBM_CUDA_TRY(cudaMalloc((void **)&h->rho0, (size_t)h->N * 4));
+        if (!h->u0) LBM_CUDA_TRY(cudaMalloc((void **)&h->u0, (size_t)h->N * 12));
+        if (h->rho0 != rho_dev) LBM_CUDA_TRY(cudaMemcpyAsync(h->rho0, rho_dev, (size_t)h->N * 4, cudaMemcpyDeviceToDevice, h->stream));
+        if (h->u0 != u_dev) LBM_CUDA_TRY(cudaMemcpyAsync(h->u0, u_dev, (size_t)h->N * 12, cudaMemcpyDeviceToDevice, h->stream));
+        r = h->rho0;
+        u = h->u0;
+    }
+    LBM_CUDA_TRY(h->ops->init(h->ddf[0], h->ddf[1], r, u, h->N, h->stream));
+    h->cur = 0;
+    h->steps = 0;
+    h->inited = true;
+    h->V = pick_cells_per_thread(h);
+    return LBM_OK;
+}
+
+int lbm_init_device(lbm_t *h, const float *rho_dev, const float *u_dev) {
+    if (int rc = enter(h)) return rc;
+    if (!rho_dev || !u_dev) return fail(LBM_E_INVAL, "lbm_init_device: rho and u must not be NULL");
+    return init_from_device(h, rho_dev, u_dev);
+}
+
+int lbm_init(lbm_t *h, const float *rho, const float *u) {
+    if (int rc = enter(h)) return rc;
+    if (!rho || !u) return fail(LBM_E_INVAL, "lbm_init: rho and u must not be NULL");
+    float *r = nullptr, *v = nullptr;
+    if (h->has_walls) {
+        if (!h->rho0) LBM_CUDA_TRY(cudaMalloc((void **)&h->rho0, (size_t)h->N * 4));
+        if (!h->u0) LBM_CUDA_TRY(cudaMalloc((void **)&h->u0, (size_t)h->N * 12));
+        r = h->rho0;
+        v = h->u0;
+    } else {
+        LBM_CUDA_TRY(cudaMalloc((void **)&r, (size_t)h->N * 4));
+        cudaError_t e = cudaMalloc((void **)&v, (size_t)h->N * 12);
+        if (e != cudaSuccess) { cudaFree(r); LBM_CUDA_TRY(e); }
+    }
+    cudaError_t e = cudaMemcpyAsync(r, rho, (size_t)h->N * 4, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(v, u, (size_t)h->N * 12, cudaMemcpyHostToDevice, h->stream);
+    int rc = LBM_OK;
+    if (e == cudaSuccess) rc = init_from_device(h, r, v);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    if (!h->has_walls) { cudaFree(r); cudaFree(v); }
+    LBM_CUDA_TRY(e);
+    if (rc) return rc;
+    LBM_CUDA_TRY(e2);
+    return LBM_OK;
+}
+
+int lbm_step(lbm_t *h, int n) {
+    if (int rc = enter(h)) return rc;
+    if (n < 0) return fail(LBM_E_INVAL, "lbm_step: n must be >= 0");
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_step: call lbm_init first");
+    const Params p = make_params(h);
+    for (int k = 0; k < n; ++k) {
+        LBM_CUDA_TRY(h->ops->stream_collide(h->ddf[h->cur], h->ddf[1 - h->cur], p, h->V, h->collision, h->has_force, h->stream));
+        h->cur = 1 - h->cur;
+        h->steps += 1;
+    }
+    return LBM_OK;
+}
+
+int lbm_read_rho_u_device(lbm_t *h, float *rho_dev, float *u_dev) {
+    if (int rc = enter(h)) return rc;
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u: call lbm_init first");
+    if (!rho_dev && !u_dev) return LBM_OK;
+    LBM_CUDA_TRY(h->ops->read(h->ddf[h->cur], make_params(h), h->has_force, rho_dev, u_dev, h->stream));
+    return LBM_OK;
+}
+
+int lbm_read_rho_u(lbm_t *h, float *rho, float *u) {
+    if (int rc = enter(h)) return rc;
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u: call lbm_init first");
+    if (!rho && !u) return LBM_OK;
+    float *d = nullptr;
+    LBM_CUDA_TRY(cudaMalloc((void **)&d, (size_t)h->N * 16));
+    cudaError_t e = h->ops->read(h->ddf[h->cur], make_params(h), h->has_force, rho ? d : nullptr, u ? d + h->N : nullptr, h->stream);
+    if (e == cudaSuccess && rho) e = cudaMemcpyAsync(rho, d, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && u) e = cudaMemcpyAsync(u, d + h->N, (size_t)h->N * 12, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    cudaFree(d);
+    LBM_CUDA_TRY(e);
+    LBM_CUDA_TRY(e2);
+    return LBM_OK;
+}
+
+int lbm_read_ddf(lbm_t *h, int i, void *out) {
+    if (int rc = enter(h)) return rc;
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_read_ddf: call lbm_init first");
+    if (i < 0 || i >= h->q || !out) return fail(LBM_E_INVAL, "lbm_read_ddf: bad direction or NULL pointer");
+    const size_t es = (size_t)elem_size(h->fmt);
+    LBM_CUDA_TRY(cudaMemcpyAsync(out, (const char *)h->ddf[h->cur] + (size_t)i * h->N * es, (size_t)h->N * es,
+                                 cudaMemcpyDeviceToHost, h->stream));
+    LBM_CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_sync(lbm_t *h) {
+    if (int rc = enter(h)) return rc;
+    LBM_CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+long long lbm_steps_done(const lbm_t *h) { return h ? h->steps : -1; }
+
+const char *lbm_kernel_name(const lbm_t *h) {
+    if (!h || !h->inited) return "";
+    return h->ops->name(h->V, h->collision, h->has_force);
+}
+
+int lbm_destroy(lbm_t *h) {
+    if (!h) return LBM_OK;
+    cudaSetDevice(h->device);
+    cudaStreamSynchronize(h->stream);
+    if (h->owns_ddf) { cudaFree(h->ddf[0]); cudaFree(h->ddf[1]); }
+    if (h->flags) cudaFree(h->flags);
+    if (h->rho0) cudaFree(h->rho0);
+    if (h->u0) cudaFree(h->u0);
+    (void)cudaGetLastError();
+    delete h;
+    return LBM_OK;
+}
+
+// ---- codecs -------------------------------------------------------------------------------------
+int lbm_codec_encode_device(int ddf_format, const float *x_dev, unsigned short *codes_dev, long long count, void *cuda_stream) {
+    if (ddf_format < LBM_FP16S || ddf_format > LBM_FP16) return fail(LBM_E_INVAL, "lbm_codec_encode: 16-bit formats only");
+    if (count < 0 || (count > 0 && (!x_dev || !codes_dev))) return fail(LBM_E_INVAL, "lbm_codec_encode: bad arguments");
+    if (count == 0) return LBM_OK;
+    LBM_CUDA_TRY(lbmk::launch_codec(ddf_format, true, x_dev, codes_dev, count, (cudaStream_t)cuda_stream));
+    return LBM_OK;
+}
+
+int lbm_codec_decode_device(int ddf_format, const unsigned short *codes_dev, float *x_dev, long long count, void *cuda_stream) {
+    if (ddf_format < LBM_FP16S || ddf_format > LBM_FP16) return fail(LBM_E_INVAL, "lbm_codec_decode: 16-bit formats only");
+    if (count < 0 || (count > 0 && (!x_dev || !codes_dev))) return fail(LBM_E_INVAL, "lbm_codec_decode: bad arguments");
+    if (count == 0) return LBM_OK;
+    LBM_CUDA_TRY(lbmk::launch_codec(ddf_format, false, codes_dev, x_dev, count, (cudaStream_t)cuda_stream));
+    return LBM_OK;
+}
+
+static int codec_host(int fmt, bool encode, const void *in, void *out, long long count) {
+    if (fmt < LBM_FP16S || fmt > LBM_FP16) return fail(LBM_E_INVAL, "lbm_codec: 16-bit formats only");
+    if (count < 0 || (count > 0 && (!in || !out))) return fail(LBM_E_INVAL, "lbm_codec: bad arguments");
+    if (count == 0) return LBM_OK;
+    const size_t in_b = (size_t)count * (encode ? 4 : 2), out_b = (size_t)count * (encode ? 2 : 4);
+    void *din = nullptr, *dout = nullptr;
+    LBM_CUDA_TRY(cudaMalloc(&din, in_b));
+    cudaError_t e = cudaMalloc(&dout, out_b);
+    if (e == cudaSuccess) e = cudaMemcpy(din, in, in_b, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = lbmk::launch_codec(fmt, encode, din, dout, count, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, out_b, cudaMemcpyDeviceToHost);
+    cudaFree(din);
+    if (dout) cudaFree(dout);
+    LBM_CUDA_TRY(e);
+    return LBM_OK;
+}
+
+int lbm_codec_encode(int ddf_format, const float *x, unsigned short *codes, long long count) {
+    return codec_host(ddf_format, true, x, codes, count);
+}
+int lbm_codec_decode(int ddf_format, const unsigned short *codes, float *x, long long count) {
+    return codec_host(ddf_format, false, codes, x, count);
+}
+
+}  // extern "C"

@@ -1,0 +1,153 @@
+// lbm_codecs.cuh -- device-side load()/store() of the DDF storage formats.
+//
+// Every decoder returns exactly the value the format's definition assigns to the code (Table 2,
+// PAPER.md:134-146; eq (7)/(8)) and every encoder returns the NEAREST
+// representable value, ties to the larger magnitude, saturating at the largest code (what the paper's
+// converters do by adding half an output ulp and truncating);
+// FP16/FP16S use the hardware binary16 conversion with round-to-nearest-even.
+// The bit manipulation below is NOT the paper's Listing 1 (written for 2021 OpenCL devices, with data
+// dependent selects and an int->float conversion as a leading-zero counter): it is re-derived for
+// sm_100a from the value definitions, branch-free on the regular domain:
+//   FP16C   decode: place the 15 magnitude bits at FP32 bits 26..12 and multiply by 2^112 (the e = 0
+//           codes become FP32 denormals, which the multiply normalises -- needs -ftz=false);
+//           encode: multiply |x| by 2^-112 rounding toward zero, add half an ulp (0x800), shift.
+//   posits  decode: one FLO (clz) gives the regime length; regime, exponent bits and fraction are
+//           merged into the FP32 word with one shift and one add (the exponent bits land on the low
+//           bits of the FP32 exponent field);
+//           encode: build the unbounded posit string "10|e|M" / "01|e|M" in a 32-bit word, one
+//           arithmetic shift by the regime length produces the run, then add-half-and-truncate.
+//           Where a long regime cuts exponent bits off, string rounding is geometric, not nearest:
+//           those slivers (|x| < 2^-33 or >= 2^19 for P16_1S, |x| < 2^-51 for P16_2C) take a rarely
+//           executed patch so that the result is the nearest value there too (R14).
+#pragma once
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+namespace lbmk {
+
+enum : int { F_FP32 = 0, F_FP16S = 1, F_FP16C = 2, F_P16_0S = 3, F_P16_1S = 4, F_P16_2C = 5, F_FP16 = 6 };
+
+template <int F>
+struct Codec;
+
+// ---- FP32: identity ---------------------------------------------------------
+template <>
+struct Codec<F_FP32> {
+    typedef float elem_t;
+    static __device__ __forceinline__ float dec(float s) { return s; }
+    static __device__ __forceinline__ float enc(float x) { return x; }
+};
+
+// ---- IEEE binary16 --------------------------------------------------------------
+template <>
+struct Codec<F_FP16> {
+    typedef unsigned short elem_t;
+    static __device__ __forceinline__ float dec(unsigned c) {
+        return __half2float(__ushort_as_half((unsigned short)c));
+    }
+    static __device__ __forceinline__ unsigned enc(float x) { return __half_as_ushort(__float2half_rn(x)); }
+};
+
+// ---- FP16S: binary16 of x * 2^15 -----------------------------------
+template <>
+struct Codec<F_FP16S> {
+    typedef unsigned short elem_t;
+    static __device__ __forceinline__ float dec(unsigned c) {
+        return __fmul_rn(__half2float(__ushort_as_half((unsigned short)c)), 3.0517578125e-5f);  // 2^-15, exact
+    }
+    static __device__ __forceinline__ unsigned enc(float x) {
+        return __half_as_ushort(__float2half_rn(__fmul_rn(x, 32768.0f)));
+    }
+};
+
+// ---- FP16C: 1-4-11, bias 15, denormals, no Inf/NaN ----------------------
+template <>
+struct Codec<F_FP16C> {
+    typedef unsigned short elem_t;
+    static __device__ __forceinline__ float dec(unsigned c) {
+        const unsigned b = ((c & 0x8000u) << 16) | ((c & 0x7FFFu) << 12);
+        return __fmul_rn(__uint_as_float(b), __uint_as_float(0x77800000u));  // * 2^112 (exact)
+    }
+    static __device__ __forceinline__ unsigned enc(float x) {
+        const unsigned xb = __float_as_uint(x);
+        const float y = __fmul_rz(__uint_as_float(xb & 0x7FFFFFFFu), __uint_as_float(0x07800000u));  // |x| * 2^-112
+        const unsigned m = min((__float_as_uint(y) + 0x800u) >> 12, 0x7FFFu);
+        return ((xb >> 16) & 0x8000u) | m;
+    }
+};
+
+// ---- two-sided posit magnitude with NE exponent bits, scaled by 2^7 --
+template <int NE>
+struct PositS {
+    static __device__ __forceinline__ float dec(unsigned c) {
+        const unsigned mm = c << 17;                        // 15-bit magnitude, top aligned
+        const int sg = (int)mm >> 31;                       // -1: regime of ones, 0: regime of zeros
+        const unsigned t = (mm ^ (unsigned)sg) | 0x10000u;  // guard bit: run length k <= 15
+        const int k = __clz((int)t);
+        const unsigned rem = mm << (k + 1);                 // exponent bit(s) + fraction, top aligned
+        const int r = (k - 1) ^ ~sg;                        // k-1 (ones) or -k (zeros)
+        // value = 2^((r << NE) + e) * (1 + F) * 2^-7; e rides on the low exponent bits of the add
+        const unsigned bits = ((unsigned)(r * (1 << NE) + 120) << 23) + (rem >> (9 - NE));
+        const unsigned sign = (c & 0x8000u) << 16;
+        return __uint_as_float((c & 0x7FFFu) ? (bits | sign) : sign);
+    }
+    static __device__ __forceinline__ unsigned enc(float x) {
+        const unsigned xb = __float_as_uint(x);
+        const unsigned Xb = __float_as_uint(__fmul_rn(__uint_as_float(xb & 0x7FFFFFFFu), 128.0f));
+        const int E = (int)(Xb >> 23) - 127;
+        const int r = E >> NE;
+        const unsigned e = (unsigned)E & ((1u << NE) - 1u);
+        const unsigned W = (r >= 0 ? 0x80000000u : 0x40000000u) | (e << (30 - NE)) | ((Xb & 0x007FFFFFu) << (7 - NE));
+        const int sh = min(r ^ (r >> 31), 31);              // r (ones run) or -r-1 (zeros run)
+        const unsigned Ws = (unsigned)((int)W >> sh);
+        unsigned code = min(((Ws >> 16) + 1u) >> 1, 0x7FFFu);
+        if (NE == 1) {
+            // exponent bit cut off by the regime: nearest-value thresholds instead of the string's
+            const unsigned LO = 0x32800000u /* 2^-26 */, HI = 0x4C800000u /* 2^26 */;
+            if (Xb - LO >= HI - LO) {
+                code = Xb < LO ? (unsigned)(Xb >= 0x31000000u /* 2^-29 */) + (unsigned)(Xb >= 0x32200000u /* 1.25*2^-27 */)
+                               : 0x7FFEu + (unsigned)(Xb >= 0x4D200000u /* 1.25*2^27 */);
+            }
+        }
+        return ((xb >> 16) & 0x8000u) | code;
+    }
+};
+template <>
+struct Codec<F_P16_0S> : PositS<0> {
+    typedef unsigned short elem_t;
+};
+template <>
+struct Codec<F_P16_1S> : PositS<1> {
+    typedef unsigned short elem_t;
+};
+
+// ---- P16_2C: regime of zeros only, 2 exponent bits, unscaled ----
+template <>
+struct Codec<F_P16_2C> {
+    typedef unsigned short elem_t;
+    static __device__ __forceinline__ float dec(unsigned c) {
+        const unsigned mm = c << 17;
+        const int r = __clz((int)(mm | 0x10000u));          // 0..15
+        const unsigned rem = mm << (r + 1);
+        const unsigned bits = ((unsigned)(124 - 4 * r) << 23) + (rem >> 7);   // 2^(e-3-4r) (1+F)
+        const unsigned sign = (c & 0x8000u) << 16;
+        return __uint_as_float((c & 0x7FFFu) ? (bits | sign) : sign);
+    }
+    static __device__ __forceinline__ unsigned enc(float x) {
+        const unsigned xb = __float_as_uint(x);
+        const unsigned Xb = xb & 0x7FFFFFFFu;
+        const int g = (int)(Xb >> 23) - 64;                 // E + 63
+        const unsigned W = 0x80000000u | (((unsigned)g & 3u) << 29) | ((Xb & 0x007FFFFFu) << 6);
+        const int r = 15 - (g >> 2);
+        unsigned code = min((((W >> (r & 31)) >> 16) + 1u) >> 1, 0x7FFFu);
+        const unsigned LO = 0x26000000u /* 2^-51 */, HI = 0x40000000u /* 2 */;
+        if (Xb - LO >= HI - LO) {
+            code = Xb >= HI ? 0x7FFFu
+                            : (unsigned)(Xb >= 0x21800000u /* 2^-60 */) + (unsigned)(Xb >= 0x23880000u /* 1.0625*2^-56 */) +
+                                  (unsigned)(Xb >= 0x24A00000u /* 1.25*2^-54 */) + (unsigned)(Xb >= 0x25A00000u /* 1.25*2^-52 */);
+        }
+        return ((xb >> 16) & 0x8000u) | code;
+    }
+};
+
+}  // namespace lbmk

@@ -1,0 +1,27 @@
+// lbm_internal.h -- host-side glue between the C ABI (lbm_api.cu) and the kernel translation units.
+// One translation unit per (velocity set, storage format) pair is compiled from lbm_unit.cu with
+// -DLBM_Q=<q> -DLBM_F=<fmt>; each exports the launchers below under a suffixed name.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "lbm_lattice.cuh"
+
+namespace lbmk {
+
+struct UnitOps {
+    // stream_collide: V cells per thread (1, 2 or 4; nx % V == 0), force = Guo term compiled in
+    cudaError_t (*stream_collide)(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st);
+    cudaError_t (*init)(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st);
+    cudaError_t (*read)(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st);
+    const char *(*name)(int V, int coll, bool force);
+};
+
+const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)
+
+// lbm_aux.cu
+cudaError_t launch_mark_near(int q, const unsigned char *in, unsigned char *out, int nx, int ny, int nz, cudaStream_t st);
+cudaError_t launch_codec(int fmt, bool encode, const void *in, void *out, long long count, cudaStream_t st);
+
+void count_launch(long long n = 1);
+
+}  // namespace lbmk

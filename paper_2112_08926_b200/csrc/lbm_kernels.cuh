@@ -1,0 +1,285 @@
+// lbm_kernels.cuh -- the fused stream-collide kernel (Listing 2; eqs (24)-(28),
+// PAPER.md:671-687) for sm_100a, templated on velocity set Q, storage format F, cells per thread V and
+// the Guo-force switch.
+//
+// What is kept from the paper: one-step pull on two buffers (reads only A, writes only B -- race free,
+// misaligned READS instead of misaligned writes), structure-of-arrays DDFs
+// (PAPER.md:939-940), DDF shifting and the operation order of the collision (section 2.2).
+// What is re-designed for B200:
+//   * no integer division or modulo: the grid is (x-tiles, y-tiles, z), the 9 neighbour rows are
+//     computed once per thread with two compares each, the wrap in x touches only the first / last
+//     cell of a row;
+//   * V consecutive cells per thread: every direction without an x component is one aligned 32/64/128-bit
+//     load, every store is one aligned vector store (the paper: one scalar per work-item);
+//   * the 18 neighbour-flag gathers of the paper's kernel are replaced by ONE private bit in the
+//     cell's own flag byte (FLAG_NEAR, written by lbm_set_flags): threads whose cells have no wall
+//     neighbour -- all of them in the benchmark box -- never touch a neighbour flag;
+//   * 64-bit element offsets (boxes beyond 608^3).
+#pragma once
+#include "lbm_lattice.cuh"
+
+namespace lbmk {
+
+// ---- raw vector access -------------------------------------------------------------------------
+template <int BYTES>
+struct Raw;
+template <>
+struct Raw<2> {
+    typedef unsigned short T;
+    static constexpr int WORDS = 1;
+    static __device__ __forceinline__ void ld(const void *p, unsigned (&w)[1]) { w[0] = __ldg((const unsigned short *)p); }
+    static __device__ __forceinline__ void st(void *p, const unsigned (&w)[1]) { *(unsigned short *)p = (unsigned short)w[0]; }
+};
+template <>
+struct Raw<4> {
+    static constexpr int WORDS = 1;
+    static __device__ __forceinline__ void ld(const void *p, unsigned (&w)[1]) { w[0] = __ldg((const unsigned *)p); }
+    static __device__ __forceinline__ void st(void *p, const unsigned (&w)[1]) { *(unsigned *)p = w[0]; }
+};
+template <>
+struct Raw<8> {
+    static constexpr int WORDS = 2;
+    static __device__ __forceinline__ void ld(const void *p, unsigned (&w)[2]) {
+        const uint2 r = __ldg((const uint2 *)p);
+        w[0] = r.x; w[1] = r.y;
+    }
+    static __device__ __forceinline__ void st(void *p, const unsigned (&w)[2]) { *(uint2 *)p = make_uint2(w[0], w[1]); }
+};
+template <>
+struct Raw<16> {
+    static constexpr int WORDS = 4;
+    static __device__ __forceinline__ void ld(const void *p, unsigned (&w)[4]) {
+        const uint4 r = __ldg((const uint4 *)p);
+        w[0] = r.x; w[1] = r.y; w[2] = r.z; w[3] = r.w;
+    }
+    static __device__ __forceinline__ void st(void *p, const unsigned (&w)[4]) { *(uint4 *)p = make_uint4(w[0], w[1], w[2], w[3]); }
+};
+
+// element <-> FP32 through the format's codec, on raw 32-bit words
+template <int F, bool IS32 = (F == F_FP32)>
+struct Elem;
+template <int F>
+struct Elem<F, true> {
+    typedef float T;
+    static constexpr int SIZE = 4;
+    static __device__ __forceinline__ float ld1(const T *p) { return __ldg(p); }
+    static __device__ __forceinline__ void st1(T *p, float x) { *p = x; }
+    template <int V>
+    static __device__ __forceinline__ float get(const unsigned (&w)[Raw<4 * V>::WORDS], int j) { return __uint_as_float(w[j]); }
+    template <int V>
+    static __device__ __forceinline__ void pack(unsigned (&w)[Raw<4 * V>::WORDS], const float (&x)[V]) {
+#pragma unroll
+        for (int j = 0; j < V; ++j) w[j] = __float_as_uint(x[j]);
+    }
+};
+template <int F>
+struct Elem<F, false> {
+    typedef unsigned short T;
+    static constexpr int SIZE = 2;
+    static __device__ __forceinline__ float ld1(const T *p) { return Codec<F>::dec((unsigned)__ldg(p)); }
+    static __device__ __forceinline__ void st1(T *p, float x) { *p = (unsigned short)Codec<F>::enc(x); }
+    template <int V>
+    static __device__ __forceinline__ float get(const unsigned (&w)[Raw<2 * V>::WORDS], int j) {
+        return Codec<F>::dec(V == 1 ? w[0] : ((j & 1) ? (w[j >> 1] >> 16) : w[j >> 1]));   // decoders ignore bits above 15
+    }
+    template <int V>
+    static __device__ __forceinline__ void pack(unsigned (&w)[Raw<2 * V>::WORDS], const float (&x)[V]) {
+        if (V == 1) {
+            w[0] = Codec<F>::enc(x[0]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < V; j += 2) w[j >> 1] = Codec<F>::enc(x[j]) | (Codec<F>::enc(x[j + 1 < V ? j + 1 : j]) << 16);
+        }
+    }
+};
+
+// ---- the pull of direction I for V consecutive cells, fast path (no wall anywhere near) ---------
+template <int Q, int F, int V, int I>
+struct PullDir {
+    typedef Elem<F> E;
+    typedef typename E::T T;
+    // rows[dy+1][dz+1] = element offset of row (y+dy, z+dz) incl. periodic wrap; x0 = first own cell;
+    // xm / xp = wrapped x0-1 / x0+V
+    static __device__ __forceinline__ void run(const T *__restrict__ A, long long N, const long long (&rows)[3][3], int x0, int xm,
+                                               int xp, float (&f)[V][Q]) {
+        typedef Lat<Q> L;
+        constexpr int cx = L::c(I, 0), cy = L::c(I, 1), cz = L::c(I, 2);
+        const T *row = A + (long long)I * N + rows[1 - cy][1 - cz];   // source row (y - cy, z - cz)
+        if (cx == 0) {
+            unsigned w[Raw<E::SIZE * V>::WORDS];
+            Raw<E::SIZE * V>::ld(row + x0, w);
+#pragma unroll
+            for (int j = 0; j < V; ++j) f[j][I] = E::template get<V>(w, j);
+        } else if (cx > 0) {                         // sources x0-1 .. x0+V-2
+            f[0][I] = E::ld1(row + xm);
+#pragma unroll
+            for (int j = 1; j < V; ++j) f[j][I] = E::ld1(row + x0 + j - 1);
+        } else {                                     // sources x0+1 .. x0+V
+#pragma unroll
+            for (int j = 0; j < V - 1; ++j) f[j][I] = E::ld1(row + x0 + j + 1);
+            f[V - 1][I] = E::ld1(row + xp);
+        }
+        PullDir<Q, F, V, I + 1>::run(A, N, rows, x0, xm, xp, f);
+    }
+};
+template <int Q, int F, int V>
+struct PullDir<Q, F, V, Q> {
+    typedef typename Elem<F>::T T;
+    static __device__ __forceinline__ void run(const T *__restrict__, long long, const long long (&)[3][3], int, int, int,
+                                               float (&)[V][Q]) {}
+};
+
+// ---- the pull of direction I for ONE cell next to a wall (R3 halfway bounce-back, R9 moving wall) --
+template <int Q, int F, int I>
+struct PullDirWall {
+    typedef Elem<F> E;
+    typedef typename E::T T;
+    static __device__ __forceinline__ void run(const T *__restrict__ A, const Params &p, const long long (&rows)[3][3], int x,
+                                               int xm, int xp, float (&f)[Q]) {
+        typedef Lat<Q> L;
+        constexpr int cx = L::c(I, 0), cy = L::c(I, 1), cz = L::c(I, 2);
+        const long long own = rows[1][1] + x;
+        if (I == 0) {
+            f[0] = E::ld1(A + own);
+        } else {
+            const long long src = rows[1 - cy][1 - cz] + (cx == 0 ? x : cx > 0 ? xm : xp);
+            if (__ldg(p.flags + src) & FLAG_WALL) {
+                float v = E::ld1(A + (long long)L::opp(I) * p.N + own);
+                const float uwx = __ldg(p.u0 + src), uwy = __ldg(p.u0 + p.N + src), uwz = __ldg(p.u0 + 2 * p.N + src);
+                if (uwx != 0.0f || uwy != 0.0f || uwz != 0.0f)       // R9, rho_w = 1
+                    v = add(v, mul(L::w6(I), cdot<Q, I>(uwx, uwy, uwz)));
+                f[I] = v;
+            } else {
+                f[I] = E::ld1(A + (long long)I * p.N + src);
+            }
+        }
+        PullDirWall<Q, F, I + 1>::run(A, p, rows, x, xm, xp, f);
+    }
+};
+template <int Q, int F>
+struct PullDirWall<Q, F, Q> {
+    typedef typename Elem<F>::T T;
+    static __device__ __forceinline__ void run(const T *__restrict__, const Params &, const long long (&)[3][3], int, int, int,
+                                               float (&)[Q]) {}
+};
+
+template <int COLL, int Q, bool FORCE>
+__device__ __forceinline__ void collide(float (&f)[Q], const Params &p) {
+    collide_bgk<Q, FORCE>(f, p);
+}
+
+constexpr int SC_THREADS = 256;
+
+// grid: x = tiles of BX*V cells along x, y = tiles of BY rows, z = plane.  blockDim = (BX, BY), BX*BY = SC_THREADS
+template <int Q, int F, int V, bool FORCE>
+__global__ void __launch_bounds__(SC_THREADS)
+stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p) {
+    typedef Elem<F> E;
+    typedef typename E::T T;
+    const int x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x0 >= p.nx || y >= p.ny) return;
+
+    // R2: periodic neighbours without modulo
+    const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
+    const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
+    const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
+    long long rows[3][3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
+    const int xm = x0 == 0 ? p.nx - 1 : x0 - 1;
+    const int xp = x0 + V >= p.nx ? 0 : x0 + V;
+    const long long own = rows[1][1] + x0;
+
+    // a1: own flags, V bytes in one load
+    static_assert(V == 1 || V == 2 || V == 4, "cells per thread");
+    unsigned any;
+    if (V == 1) any = __ldg(p.flags + own);
+    else if (V == 2) any = __ldg((const unsigned short *)(p.flags + own));
+    else any = __ldg((const unsigned *)(p.flags + own));
+
+    float f[V][Q];
+    if (any == 0) {
+        // ---- fast path: a3 load + decode, a5-a9 collide, a10 encode + store, all vectorised --------
+        PullDir<Q, F, V, 0>::run(A, p.N, rows, x0, xm, xp, f);
+#pragma unroll
+        for (int j = 0; j < V; ++j) collide<0, Q, FORCE>(f[j], p);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            float o[V];
+#pragma unroll
+            for (int j = 0; j < V; ++j) o[j] = f[j][i];
+            unsigned w[Raw<E::SIZE * V>::WORDS];
+            E::template pack<V>(w, o);
+            Raw<E::SIZE * V>::st(B + (long long)i * p.N + own, w);
+        }
+    } else {
+        // ---- a wall cell or a wall neighbour in this thread's cells: cell by cell ------------------
+#pragma unroll 1
+        for (int j = 0; j < V; ++j) {
+            if ((any >> (8 * j)) & FLAG_WALL) continue;
+            const int x = x0 + j;
+            const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
+            float g[Q];
+            PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, g);
+            collide<0, Q, FORCE>(g, p);
+#pragma unroll
+            for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + own + j, g[i]);
+        }
+    }
+}
+
+// ---- init: every cell, walls included, both buffers (R11) -----------------------
+template <int Q, int F>
+__global__ void __launch_bounds__(256)
+init_kernel(typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const float *__restrict__ rho,
+            const float *__restrict__ u, long long N) {
+    typedef Elem<F> E;
+    for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
+        float feq[Q];
+        equilibrium<Q>(__ldg(rho + n), __ldg(u + n), __ldg(u + N + n), __ldg(u + 2 * N + n), feq);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            unsigned w[1];
+            const float o[1] = {feq[i]};
+            E::template pack<1>(w, o);
+            Raw<E::SIZE>::st(A + (long long)i * N + n, w);
+            Raw<E::SIZE>::st(B + (long long)i * N + n, w);
+        }
+    }
+}
+
+// ---- read-out: local moments of the current buffer (R12) -------------------------------------------
+template <int Q, int F, bool FORCE>
+__global__ void __launch_bounds__(256)
+read_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, float *__restrict__ rho_out,
+                  float *__restrict__ u_out) {
+    typedef Elem<F> E;
+    const long long N = p.N;
+    for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
+        float rho, j[3], u[3];
+        if (__ldg(p.flags + n) & FLAG_WALL) {
+            rho = __ldg(p.rho0 + n);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) u[a] = __ldg(p.u0 + a * N + n);
+        } else {
+            float f[Q];
+#pragma unroll
+            for (int i = 0; i < Q; ++i) f[i] = E::ld1(A + (long long)i * N + n);
+            moments<Q>(f, rho, j);
+            const float Fv[3] = {p.fx, p.fy, p.fz};
+#pragma unroll
+            for (int a = 0; a < 3; ++a) u[a] = __fdiv_rn(FORCE ? fma_(-0.5f, Fv[a], j[a]) : j[a], rho);
+        }
+        if (rho_out) rho_out[n] = rho;
+        if (u_out) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) u_out[a * N + n] = u[a];
+        }
+    }
+}
+
+}  // namespace lbmk

@@ -1,0 +1,84 @@
+// lbm_unit.cu -- one (velocity set, storage format) instantiation unit of the kernels in
+// lbm_kernels.cuh.  Compiled once per pair with -DLBM_Q=<9|19|27> -DLBM_F=<0..6> (see build.py).
+#include "lbm_internal.h"
+#include "lbm_kernels.cuh"
+
+#ifndef LBM_Q
+#error "compile with -DLBM_Q=<velocity set> -DLBM_F=<format>"
+#endif
+
+#define LBM_CAT_(a, b, c, d) a##b##c##d
+#define LBM_CAT(a, b, c, d) LBM_CAT_(a, b, c, d)
+#define LBM_UNIT_SYMBOL LBM_CAT(lbm_unit_q, LBM_Q, _f, LBM_F)
+#define LBM_STR_(x) #x
+#define LBM_STR(x) LBM_STR_(x)
+
+namespace lbmk {
+namespace {
+
+constexpr int Q = LBM_Q, F = LBM_F;
+typedef typename Elem<F>::T T;
+
+template <int V, bool FORCE>
+cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) {
+    const int tx = (p.nx + V - 1) / V;
+    int bx = 1;
+    while (bx < tx && bx < SC_THREADS) bx <<= 1;
+    const int by = SC_THREADS / bx;
+    const dim3 block(bx, by, 1);
+    const dim3 grid((tx + bx - 1) / bx, (p.ny + by - 1) / by, p.nz);
+    stream_collide_kernel<Q, F, V, FORCE><<<grid, block, 0, st>>>((const T *)A, (T *)B, p);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
+    (void)coll;
+    switch (V * 2 + (force ? 1 : 0)) {
+        case 2: return launch_sc<1, false>(A, B, p, st);
+        case 3: return launch_sc<1, true>(A, B, p, st);
+        case 4: return launch_sc<2, false>(A, B, p, st);
+        case 5: return launch_sc<2, true>(A, B, p, st);
+        case 8: return launch_sc<4, false>(A, B, p, st);
+        case 9: return launch_sc<4, true>(A, B, p, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+int blocks_for(long long N) {
+    long long b = (N + 255) / 256;
+    const long long cap = 148LL * 64;   // grid-stride loops: a few waves over the 148 SMs
+    return (int)(b < cap ? (b < 1 ? 1 : b) : cap);
+}
+
+cudaError_t init(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st) {
+    init_kernel<Q, F><<<blocks_for(N), 256, 0, st>>>((T *)A, (T *)B, rho, u, N);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t read(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st) {
+    if (force) read_rho_u_kernel<Q, F, true><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
+    else read_rho_u_kernel<Q, F, false><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
+    count_launch();
+    return cudaGetLastError();
+}
+
+const char *name(int V, int coll, bool force) {
+    (void)coll;
+    static const char *names[3][2] = {
+        {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=0>",
+         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=1>"},
+        {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=0>",
+         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=1>"},
+        {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=0>",
+         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=1>"}};
+    return names[V == 1 ? 0 : V == 2 ? 1 : 2][force ? 1 : 0];
+}
+
+}  // namespace
+
+extern const UnitOps LBM_UNIT_SYMBOL;
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name};
+
+}  // namespace lbmk
