@@ -1,0 +1,75 @@
+"""GPU: C-ABI behaviour of liblbm_b200.so -- argument checks, call-order rules, ownership."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import paper_2112_08926_b200 as lbm
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def test_create_rejects_bad_arguments():
+    for kw, code in [(dict(nx=0), lbm.E_INVAL), (dict(velset=7), lbm.E_INVAL), (dict(tau=0.5), lbm.E_INVAL),
+                     (dict(ddf_format=9), lbm.E_INVAL), (dict(collision=lbm.TRT), lbm.E_UNSUPPORTED),
+                     (dict(velset=9, nz=2), lbm.E_INVAL)]:
+        args = dict(nx=8, ny=8, nz=8, velset=19, ddf_format=0, tau=0.6, collision=0)
+        args.update(kw)
+        with pytest.raises(lbm.LbmError) as e:
+            lbm.Simulation(args["nx"], args["ny"], args["nz"], args["velset"], args["ddf_format"], args["tau"],
+                           collision=args["collision"])
+        assert e.value.code == code
+        assert lbm.last_error()
+
+
+def test_call_order_and_flags_validation():
+    s = lbm.Simulation(8, 4, 4, 19, "FP16S", 0.6)
+    with pytest.raises(lbm.LbmError) as e:
+        s.step(1)
+    assert e.value.code == lbm.E_STATE
+    with pytest.raises(lbm.LbmError) as e:
+        s.set_flags(np.full(128, 2, np.uint8))
+    assert e.value.code == lbm.E_INVAL
+    s.init(np.ones(128, np.float32), np.zeros((3, 128), np.float32))
+    with pytest.raises(lbm.LbmError) as e:
+        s.set_flags(np.zeros(128, np.uint8))
+    assert e.value.code == lbm.E_STATE
+    with pytest.raises(lbm.LbmError):
+        s.step(-1)
+    s.step(0)
+    assert s.steps_done == 0
+    s.step(3)
+    assert s.steps_done == 3
+    rho, u = s.read_rho_u()
+    assert np.all(rho == 1.0) and np.all(u == 0.0)          # rest state is a fixed point
+    for i in range(19):
+        assert np.all((s.read_ddf(i) & 0x7FFF) == 0)        # codes 0x0000 / 0x8000 only
+    s.close()
+
+
+def test_library_owned_memory_and_device_io_agree_with_torch_memory():
+    import torch
+    w = wl.perturbed_equilibrium(20, 6, 4, seed=2)
+    a = lbm.from_workload(w, "FP16C")                       # torch-owned DDF buffers, host init
+    b = lbm.Simulation(w.nx, w.ny, w.nz, 19, "FP16C", w.tau, use_torch_memory=False)
+    b.init(torch.from_numpy(w.rho).cuda(), torch.from_numpy(w.u).cuda())   # library-owned, device init
+    a.step(7)
+    b.step(7)
+    ra, ua = a.read_rho_u()
+    rb, ub = b.read_rho_u_device()
+    assert np.array_equal(ra, rb.cpu().numpy()) and np.array_equal(ua, ub.cpu().numpy())
+
+
+def test_launch_counter_counts_kernels():
+    w = wl.perturbed_equilibrium(16, 4, 4, seed=2)
+    s = lbm.from_workload(w, "FP32")
+    n0 = lbm.launch_count()
+    s.step(5)
+    assert lbm.launch_count() - n0 == 5
+
+
+def test_sizes():
+    assert lbm.bytes_per_cell(19, "FP32") == 153 and lbm.bytes_per_cell(19, "FP16S") == 77
+    assert lbm.bytes_per_cell(27, "FP32") == 217 and lbm.bytes_per_cell(9, "P16_2C") == 37
+    assert lbm.ddf_buffer_bytes(32, 32, 32, 19, "FP16C") == 32 ** 3 * 19 * 2
