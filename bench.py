@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPs/s and HBM-roofline fraction of the fused LBM stream-collide step on B200.
+
+Workload (BASELINE.json configs[4], the paper's own benchmark box): D3Q19, BGK, fully
+periodic cube L^3 (default 512^3, far beyond the 126 MB L2) with no boundary nodes, perturbed-equilibrium
+initial state (workloads.perturbed_equilibrium, seeded).  A "step" is one lbm_step(1): one launch of the
+fused stream_collide kernel over the whole box.  The metric is BASELINE.json's: D3Q19 MLUPs/s per DDF
+storage format and achieved HBM GB/s vs the measured peak.  The JSON line's `value` is the headline
+format (FP16S, the paper's fastest); every format is listed under `formats`.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size L] [--formats FP32,FP16S,...]
+    python bench.py --impl reference     # the CPU oracle, as it stands, on a bounded sample
+
+N > 1 (torchrun): the path does not exchange data between GPUs in this tier:
+every rank runs an independent replica of the box ("weak" scaling), timed as the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "D3Q19 MLUPs/s per DDF format (headline: FP32 arithmetic / FP16S storage); HBM GB/s vs peak"
+HEADLINE = "FP16S"
+SEED = 20211208
+TAU = 0.6
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def recorded_traffic(fmt_name, size):
+    """DRAM bytes per launch from the committed ncu --set full capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        d = json.load(open(path))
+        e = d.get(f"D3Q19_{fmt_name}_{size}")
+        return None if e is None else float(e["dram_bytes_per_launch"])
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+
+    def summary(self, windows):
+        sm, smax, reasons, power = [], 0.0, set(), 0.0
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, line in self.rows:
+            if not any(a <= t <= b for a, b in windows):
+                continue
+            p = [s.strip() for s in line.split(",")]
+            try:
+                sm.append(float(p[0])); smax = max(smax, float(p[1])); power = max(power, float(p[2]))
+            except Exception:
+                continue
+            for n, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax or None,
+                "power_w_max": power or None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_setup(n_gpus):
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        import torch
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    return world, rank, local
+
+
+def run_ours(args):
+    import torch
+
+    import paper_2112_08926_b200 as lbm
+
+    world, rank, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+    L, K, W = args.size, args.steps, args.warmup
+    N = L ** 3
+    formats = args.formats.split(",")
+    peak, peak_src = measured_peak()
+
+    # synthetic input, host side (pinned, for the end-to-end leg) and a device copy
+    w = wl.perturbed_equilibrium(L, L, L, seed=SEED + rank, tau=TAU)
+    rho_h = torch.from_numpy(w.rho).pin_memory()
+    u_h = torch.from_numpy(w.u).pin_memory()
+    rho_d, u_d = rho_h.cuda(), u_h.cuda()
+    rho_out = torch.empty(N, dtype=torch.float32).pin_memory()
+    u_out = torch.empty((3, N), dtype=torch.float32).pin_memory()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    windows = []
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if dist is None:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    results, launches_total = {}, 0
+    for name in formats:
+        sim = lbm.Simulation(L, L, L, 19, name, TAU, cells_per_thread=args.cells_per_thread)
+        sim.init(rho_d, u_d)
+        sim.step(W)
+        barrier()
+        n0 = lbm.launch_count()
+        t0 = sampler.mark()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        sim.step(K)                       # K launches of stream_collide on torch's current stream
+        e1.record()
+        barrier()
+        windows.append((t0, sampler.mark()))
+        ms = max_over_ranks(e0.elapsed_time(e1))
+        launches = lbm.launch_count() - n0
+        launches_total += launches
+        rho_chk, _ = sim.read_rho_u_device()
+        assert bool(torch.isfinite(rho_chk).all()), name
+        # end to end through the public API with HOST buffers: init (H2D) + K steps + read-out (D2H)
+        barrier()
+        t_e2e = time.perf_counter()
+        sim.init(rho_h.numpy(), u_h.numpy())
+        sim.step(K)
+        sim.read_rho_u(out=(rho_out.numpy(), u_out.numpy()))
+        torch.cuda.synchronize()
+        e2e_ms = max_over_ranks((time.perf_counter() - t_e2e) * 1e3)
+        bpc = lbm.bytes_per_cell(19, name)
+        mlups = world * N * K / (ms * 1e-3) / 1e6
+        gbs = N * bpc / (ms / K * 1e-3) / 1e9         # per GPU, per launch
+        results[name] = {"mlups": round(mlups, 1), "ms_per_step": round(ms / K, 4), "bytes_per_cell": bpc,
+                         "hbm_gbs": round(gbs, 1), "frac_of_peak": round(gbs / peak, 4),
+                         "e2e_mlups": round(world * N * K / (e2e_ms * 1e-3) / 1e6, 1), "kernel": sim.kernel_name,
+                         "launches": launches}
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    sampler.stop()
+    if rank != 0:
+        return
+    head = HEADLINE if HEADLINE in results else formats[0]
+    r = results[head]
+    clocks = sampler.summary(windows)
+    line = {
+        "metric": METRIC, "value": r["mlups"], "unit": "MLUPs/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[4] bandwidth sweep: D3Q19 BGK periodic cube {L}^3, perturbed equilibrium "
+                               f"(seed {SEED}), tau {TAU}, headline storage format {head}",
+                   "cells": N, "l2_policy": "inputs larger than L2 (two DDF buffers of "
+                                            f"{N * 19 * (4 if head == 'FP32' else 2) / 1e9:.1f} GB each, no flush needed)",
+                   "parallelism": f"{world} independent replica(s)"},
+        "formats": results,
+        "speedup_16bit_vs_fp32": (round(results[head]["mlups"] / results["FP32"]["mlups"], 3)
+                                  if "FP32" in results and head != "FP32" else None),
+        "roofline": {"bound": "hbm", "kernel": r["kernel"], "achieved": r["hbm_gbs"], "peak": peak, "unit": "GB/s",
+                     "frac": r["frac_of_peak"], "traffic": recorded_traffic(head, L), "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": N * r["bytes_per_cell"]},
+        "e2e": {"value": r["e2e_mlups"], "unit": "MLUPs/s", "h2d_bytes_per_step": 16 * N / K,
+                "d2h_bytes_per_step": 16 * N / K,
+                "what": f"lbm_init(host rho,u) + lbm_step({K}) + lbm_read_rho_u(host), wall clock, pinned host buffers"},
+        "gpu_launches": launches_total, "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(head, budget_s=args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def oracle_run(fmt_name, L, steps, warmup):
+    """Time the CPU oracle, as it stands, on an L^3 sample of the workload.  Returns (mlups, cores, seconds)."""
+    import oracle
+    cores = oracle.set_threads(os.cpu_count() or 1)
+    w = wl.perturbed_equilibrium(L, L, L, seed=SEED, tau=TAU)
+    sim = oracle.from_workload(w, wl.FORMATS[fmt_name])
+    sim.step(warmup)
+    t0 = time.perf_counter()
+    sim.step(steps)
+    dt = time.perf_counter() - t0
+    return L ** 3 * steps / dt / 1e6, cores, dt
+
+
+def cpu_baseline(fmt_name, budget_s=15.0):
+    """The oracle on a BOUNDED sample: a 128^3 periodic box of the same recipe (beyond the LLC), step
+    count sized from a 1-step probe so that the timed part takes about `budget_s` seconds."""
+    L = 128
+    probe, cores, dt = oracle_run(fmt_name, L, 1, 1)
+    steps = max(2, min(200, int(budget_s / max(dt, 1e-3))))
+    mlups, cores, dt = oracle_run(fmt_name, L, steps, 0)
+    return {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle",
+            "sample": f"D3Q19 BGK {fmt_name} storage, {L}^3 periodic box of the same recipe, {steps} steps, {dt:.1f} s"}
+
+
+def run_reference(args):
+    """--impl reference: for this tier the reference arm is the CPU oracle (there is no reference code)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    K, W = args.steps, args.warmup
+    L = 128
+    probe, cores, dt1 = oracle_run(HEADLINE, L, 1, 0)
+    K_eff = max(1, min(K, int(120.0 / max(dt1, 1e-3))))       # keep the whole run within a few minutes
+    mlups, cores, dt = oracle_run(HEADLINE, L, K_eff, min(W, 2))
+    sample = (f"D3Q19 BGK {HEADLINE} storage, {L}^3 periodic sample box of the {args.size}^3 workload, "
+              f"{K_eff} timed steps, {dt:.1f} s, {cores} OpenMP threads")
+    line = {"impl": "reference", "metric": METRIC, "value": round(mlups, 2), "unit": "MLUPs/s",
+            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": K_eff, "warmup": min(W, 2),
+            "ms_per_step": round(dt / K_eff * 1e3, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"configs[4] bandwidth sweep: D3Q19 BGK periodic cube, perturbed equilibrium "
+                                   f"(seed {SEED}), tau {TAU}, storage format {HEADLINE}; CPU oracle on a bounded sample",
+                       "sample": sample},
+            "cpu_baseline": {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": round(mlups, 2), "unit": "MLUPs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--size", type=int, default=512, help="cube edge L")
+    ap.add_argument("--formats", default="FP32,FP16S,FP16C,P16_0S,P16_1S,P16_2C")
+    ap.add_argument("--cells-per-thread", type=int, default=0, help="0 = library default")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
