@@ -49,16 +49,21 @@ def measured_peak():
 
 
 def recorded_traffic(fmt_name, size):
-    """DRAM bytes per launch from the committed ncu --set full capture (profiles/), or None."""
-    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the stream_collide kernel from the
+    committed `ncu --set full` capture: profiles/dram_traffic.csv, columns velset,format,L,bytes_per_launch,profile.
+    The LAST matching row wins (newest profile).  None if no capture exists for this format / size."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
         return None
-    try:
-        d = json.load(open(path))
-        e = d.get(f"D3Q19_{fmt_name}_{size}")
-        return None if e is None else float(e["dram_bytes_per_launch"])
-    except Exception:
-        return None
+    found = None
+    for line in open(path):
+        p = [c.strip() for c in line.split(",")]
+        if len(p) >= 4 and p[0] == "D3Q19" and p[1] == fmt_name and p[2] == str(size):
+            try:
+                found = float(p[3])
+            except ValueError:
+                pass
+    return found
 
 
 class ClockSampler:
