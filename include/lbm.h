@@ -69,8 +69,15 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, i
  * cast to void* (NULL = the legacy default stream).  Must be called before lbm_init. */
 int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream);
 
-/* Tuning knob: cells per thread of the stream_collide kernel, v in {0 = automatic, 1, 2, 4}; nx must be
- * a multiple of v.  The result of a run does not depend on it (tests check that bit for bit). */
+/* Tuning knob: which stream_collide kernel runs.  The result of a run does not depend on it (tests check that
+ * bit for bit).
+ *   LBM_VARIANT_AUTO   the library chooses;
+ *   1, 2, 4            the per-thread kernel with that many cells per thread along x (nx a multiple of it);
+ *   LBM_VARIANT_BULK   the shared-memory-staged kernel: DDF rows move by cp.async.bulk, persistent CTAs
+ *                      (nx a multiple of 16).
+ * lbm_set_cells_per_thread(h, v) = lbm_set_variant(h, v) restricted to v in {0, 1, 2, 4}. */
+enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16 };
+int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_cells_per_thread(lbm_t *h, int v);
 
 /* Set the cell flags.  flags: HOST pointer, N bytes, copied.  Only LBM_FLAG_WALL may be set
@@ -119,6 +126,11 @@ int lbm_codec_encode_device(int ddf_format, const float *x_dev, unsigned short *
                             void *cuda_stream);
 int lbm_codec_decode_device(int ddf_format, const unsigned short *codes_dev, float *x_dev, long long count,
                             void *cuda_stream);
+
+/* Device self-check of the staged kernel's pair converters against the scalar converters above: all 65 536 codes
+ * through the pair decoders and all 2^32 FP32 bit patterns through the pair encoder, compared bit for bit (NaN
+ * inputs excepted).  *mismatches (HOST) receives the number of differences (0 = identical).  Synchronous. */
+int lbm_codec_pair_selftest(int ddf_format, long long *mismatches);
 
 /* ---- sizes -------------------------------------------------------------------------------------*/
 /* bytes of ONE DDF buffer: q * N * sizeof(element), rounded up to a multiple of 256 */

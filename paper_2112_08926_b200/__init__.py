@@ -28,6 +28,7 @@ BGK, TRT = 0, 1
 FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C": 5, "FP16": 6}
 FORMAT_NAMES = {v: k for k, v in FORMATS.items()}
 FLAG_WALL = 0x01
+VARIANT_AUTO, VARIANT_BULK = 0, 16
 OK, E_INVAL, E_UNSUPPORTED, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/lbm.h declares: (restype, argtypes)
@@ -35,6 +36,7 @@ _p, _i, _ll, _f = C.c_void_p, C.c_int, C.c_longlong, C.c_float
 SYMBOLS = {
     "lbm_create": (_i, [C.POINTER(_p), _i, _i, _i, _i, _i, _i, _f, _p]),
     "lbm_bind": (_i, [_p, _p, _p, _p]),
+    "lbm_set_variant": (_i, [_p, _i]),
     "lbm_set_cells_per_thread": (_i, [_p, _i]),
     "lbm_set_flags": (_i, [_p, _p]),
     "lbm_init": (_i, [_p, _p, _p]),
@@ -51,6 +53,7 @@ SYMBOLS = {
     "lbm_codec_decode": (_i, [_i, _p, _p, _ll]),
     "lbm_codec_encode_device": (_i, [_i, _p, _p, _ll, _p]),
     "lbm_codec_decode_device": (_i, [_i, _p, _p, _ll, _p]),
+    "lbm_codec_pair_selftest": (_i, [_i, C.POINTER(_ll)]),
     "lbm_ddf_buffer_bytes": (_ll, [_i, _i, _i, _i, _i]),
     "lbm_bytes_per_cell": (_ll, [_i, _i]),
     "lbm_kernel_name": (C.c_char_p, [_p]),
@@ -119,7 +122,7 @@ class Simulation:
     """One LBM box on the current CUDA device.  Mirrors the C ABI call for call."""
 
     def __init__(self, nx, ny, nz, velset=D3Q19, ddf_format="FP32", tau=0.6, force=None, collision=BGK,
-                 use_torch_memory=True, cells_per_thread=0):
+                 use_torch_memory=True, cells_per_thread=0, variant=0):
         self._h = C.c_void_p()
         self.nx, self.ny, self.nz, self.q = int(nx), int(ny), int(nz), int(velset)
         self.N = self.nx * self.ny * self.nz
@@ -142,6 +145,8 @@ class Simulation:
             _check(lib().lbm_bind(self._h, a.data_ptr(), b.data_ptr(), stream))
         if cells_per_thread:
             _check(lib().lbm_set_cells_per_thread(self._h, int(cells_per_thread)))
+        if variant:
+            _check(lib().lbm_set_variant(self._h, int(variant)))
 
     # -- lifetime ------------------------------------------------------------------------------
     def close(self):
@@ -165,6 +170,9 @@ class Simulation:
     # -- the ABI -------------------------------------------------------------------------------
     def set_cells_per_thread(self, v: int):
         _check(lib().lbm_set_cells_per_thread(self._h, int(v)))
+
+    def set_variant(self, v: int):
+        _check(lib().lbm_set_variant(self._h, int(v)))
 
     def set_flags(self, flags):
         flags = np.ascontiguousarray(flags, dtype=np.uint8).reshape(-1)
@@ -250,3 +258,11 @@ def codec_decode(ddf_format, codes) -> np.ndarray:
     out = np.empty(codes.shape, np.float32)
     _check(lib().lbm_codec_decode(_fmt(ddf_format), _np_ptr(codes), _np_ptr(out), codes.size))
     return out
+
+
+def codec_pair_selftest(ddf_format) -> int:
+    """Number of bit mismatches between the staged kernel's pair converters and the scalar converters,
+    exhaustive over all codes / all FP32 patterns, computed on the GPU (0 = identical)."""
+    n = _ll(0)
+    _check(lib().lbm_codec_pair_selftest(_fmt(ddf_format), C.byref(n)))
+    return int(n.value)

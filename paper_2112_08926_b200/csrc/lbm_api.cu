@@ -33,8 +33,8 @@ struct lbm {
     float *rho0, *u0;          // device copies of the init fields, kept only when the box has walls
     long long steps;
     bool inited;
-    int V;                     // cells per thread of the stream_collide variant in use
-    int V_request;             // 0 = automatic
+    int V;                     // stream_collide variant in use: 1, 2, 4 cells per thread or LBM_VARIANT_BULK
+    int V_request;             // LBM_VARIANT_AUTO = automatic
     const UnitOps *ops;
 };
 
@@ -98,16 +98,20 @@ int ensure_ddf(lbm *h) {
     return LBM_OK;
 }
 
-// cells per thread: the widest of {4, 2, 1} that divides nx (vector loads must not straddle a row);
-// the per-format default comes from the bandwidth sweep recorded in DESIGN.md section 5
-int pick_cells_per_thread(const lbm *h) {
+// Kernel variant.  Automatic choice: the shared-memory-staged kernel (lbm_bulk.cuh) for every 16-bit format
+// when rows are 16-cell aligned and at least half a tile long -- it is what lifts the 16-bit formats out of
+// the issue bound; FP32 storage stays on the per-thread kernel, which already runs at
+// the HBM roofline.  Per-thread kernel: the widest of {2, 1} cells per thread that divides nx.
+int pick_variant(const lbm *h) {
     int want = h->V_request;
     if (want == 0) {
-        const char *env = getenv("LBM_CELLS_PER_THREAD");
+        const char *env = getenv("LBM_VARIANT");
         if (env && *env) want = atoi(env);
     }
-    if (want == 0) want = 2;
-    if (want != 1 && want != 2 && want != 4) want = 1;
+    const bool bulk_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->bulk_tile_cells() - 1) / h->ops->bulk_tile_cells()) * h->ny * h->nz <= 0x7FFFFFFFLL;
+    if (want == LBM_VARIANT_BULK && bulk_ok) return LBM_VARIANT_BULK;
+    if (want == 0 && bulk_ok && h->fmt != LBM_FP32 && 2 * h->nx >= h->ops->bulk_tile_cells()) return LBM_VARIANT_BULK;
+    if (want != 1 && want != 2 && want != 4) want = 2;
     while (want > 1 && h->nx % want != 0) want >>= 1;
     return want;
 }
@@ -190,13 +194,21 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream) {
     return LBM_OK;
 }
 
-int lbm_set_cells_per_thread(lbm_t *h, int v) {
+int lbm_set_variant(lbm_t *h, int v) {
     if (int rc = enter(h)) return rc;
-    if (v != 0 && v != 1 && v != 2 && v != 4) return fail(LBM_E_INVAL, "lbm_set_cells_per_thread: 0 (auto), 1, 2 or 4");
-    if (v > 1 && h->nx % v != 0) return fail(LBM_E_INVAL, "lbm_set_cells_per_thread: nx must be a multiple of v");
+    if (v != LBM_VARIANT_AUTO && v != 1 && v != 2 && v != 4 && v != LBM_VARIANT_BULK)
+        return fail(LBM_E_INVAL, "lbm_set_variant: 0 (auto), 1, 2, 4 (cells per thread) or LBM_VARIANT_BULK");
+    if ((v == 2 || v == 4) && h->nx % v != 0) return fail(LBM_E_INVAL, "lbm_set_variant: nx must be a multiple of the cells per thread");
+    if (v == LBM_VARIANT_BULK && h->nx % 16 != 0) return fail(LBM_E_INVAL, "lbm_set_variant: the staged kernel needs nx to be a multiple of 16");
     h->V_request = v;
-    h->V = pick_cells_per_thread(h);
+    h->V = pick_variant(h);
+    if (v == LBM_VARIANT_BULK && h->V != v) return fail(LBM_E_INVAL, "lbm_set_variant: box too large for the staged kernel's tile index");
     return LBM_OK;
+}
+
+int lbm_set_cells_per_thread(lbm_t *h, int v) {
+    if (v != 0 && v != 1 && v != 2 && v != 4) return fail(LBM_E_INVAL, "lbm_set_cells_per_thread: 0 (auto), 1, 2 or 4");
+    return lbm_set_variant(h, v);
 }
 
 int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
@@ -239,7 +251,7 @@ static int init_from_device(lbm *h, const float *rho_dev, const float *u_dev) {
     h->cur = 0;
     h->steps = 0;
     h->inited = true;
-    h->V = pick_cells_per_thread(h);
+    h->V = pick_variant(h);
     return LBM_OK;
 }
 
@@ -388,6 +400,19 @@ int lbm_codec_encode(int ddf_format, const float *x, unsigned short *codes, long
 }
 int lbm_codec_decode(int ddf_format, const unsigned short *codes, float *x, long long count) {
     return codec_host(ddf_format, false, codes, x, count);
+}
+
+int lbm_codec_pair_selftest(int ddf_format, long long *mismatches) {
+    if (ddf_format < LBM_FP16S || ddf_format > LBM_FP16 || !mismatches) return fail(LBM_E_INVAL, "lbm_codec_pair_selftest: bad arguments");
+    unsigned long long *d = nullptr, hval = 0;
+    LBM_CUDA_TRY(cudaMalloc((void **)&d, 8));
+    cudaError_t e = cudaMemset(d, 0, 8);
+    if (e == cudaSuccess) e = lbmk::launch_pair_selftest(ddf_format, d, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(&hval, d, 8, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    LBM_CUDA_TRY(e);
+    *mismatches = (long long)hval;
+    return LBM_OK;
 }
 
 }  // extern "C"

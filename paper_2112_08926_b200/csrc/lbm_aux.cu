@@ -82,4 +82,53 @@ cudaError_t launch_codec(int fmt, bool encode, const void *in, void *out, long l
     return cudaErrorInvalidValue;
 }
 
+// ---- pair codecs vs scalar codecs, exhaustively, on the device ----------------------------------------
+// PairCodec<F> (the staged kernel's converters) must return bit for bit what Codec<F> returns (times 2^SC):
+// all 65 536 codes through dec1 / dec2 (both halves) and ALL 2^32 FP32 bit patterns through enc2 (both halves).
+// Codec<F> itself is compared with the oracle by the tests; this closes the chain for PairCodec<F>.
+template <int F>
+__global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *mismatches) {
+    typedef PairCodec<F> PC;
+    const float up = pow2f(PC::SC);
+    unsigned long long bad = 0;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long v = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; v < (1ull << 32); v += stride) {
+        const unsigned b = (unsigned)v;
+        const float x = __uint_as_float(b);
+        const float other = __uint_as_float(b * 2654435761u + 12345u);          // an unrelated partner value
+        const unsigned ref = Codec<F>::enc(x), ref_o = Codec<F>::enc(other);
+        const unsigned w1 = PC::enc2(__fmul_rn(x, up), __fmul_rn(other, up));
+        const unsigned w2 = PC::enc2(__fmul_rn(other, up), __fmul_rn(x, up));
+        const bool nan = x != x || other != other;                              // NaN payloads of binary16 are not pinned
+        if (!nan) bad += (w1 != (ref | (ref_o << 16))) + (w2 != (ref_o | (ref << 16)));
+        if (v < 65536) {
+            const unsigned c = (unsigned)v, c2 = (c * 40503u + 7u) & 0xFFFFu;
+            const float r = __fmul_rn(Codec<F>::dec(c), up), r2 = __fmul_rn(Codec<F>::dec(c2), up);
+            float a, d;
+            PC::dec2(c | (c2 << 16), a, d);
+            const float e = PC::dec1((int)(short)c);
+            const bool cn = r != r || r2 != r2;
+            if (cn) bad += !(a != a || !(r != r)) + !(d != d || !(r2 != r2)) + !(e != e || !(r != r));
+            else bad += (__float_as_uint(a) != __float_as_uint(r)) + (__float_as_uint(d) != __float_as_uint(r2)) +
+                        (__float_as_uint(e) != __float_as_uint(r));
+        }
+    }
+    if (bad) atomicAdd(mismatches, bad);
+}
+
+cudaError_t launch_pair_selftest(int fmt, unsigned long long *mismatches_dev, cudaStream_t st) {
+    const int blocks = 148 * 16;
+    switch (fmt) {
+        case F_FP16S: pair_selftest_kernel<F_FP16S><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        case F_FP16C: pair_selftest_kernel<F_FP16C><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        case F_P16_0S: pair_selftest_kernel<F_P16_0S><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        case F_P16_1S: pair_selftest_kernel<F_P16_1S><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        case F_P16_2C: pair_selftest_kernel<F_P16_2C><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        case F_FP16: pair_selftest_kernel<F_FP16><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        default: return cudaErrorInvalidValue;
+    }
+    count_launch();
+    return cudaGetLastError();
+}
+
 }  // namespace lbmk

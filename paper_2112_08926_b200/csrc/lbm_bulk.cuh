@@ -1,0 +1,300 @@
+// lbm_bulk.cuh -- the shared-memory-staged stream-collide kernel for sm_100a: the same time step as
+// stream_collide_kernel (Listing 2; eqs (24)-(28)), with the DDF
+// streams moved by the bulk-copy engine (cp.async.bulk, SASS UBLKCP) instead of per-thread loads and stores.
+//
+// Why (profiles/r01a_first_path.md): with per-thread LDG/STG every 16-bit format is issue-bound on B200, and
+// the largest single item is 64-bit address arithmetic -- 19 streams x (base + i*N + row + x) per thread.  In
+// a structure-of-arrays pull step every direction of a row of cells is ONE contiguous segment of ONE source
+// row (eq (24)), so a tile needs q plain 1-D copies; once the segments sit in shared
+// memory every address is "thread base + compile-time immediate".
+//
+// Shape of the kernel
+//   * persistent CTAs (grid = SMs x resident CTAs), tiles handed out round-robin; a tile is up to TX = 2*NT
+//     consecutive cells of one row (y, z); NT consumer threads handle two neighbouring cells each;
+//   * warp 0 moves the data: lane i < q issues the copy of direction i -- TX elements of source row
+//     (y - c_iy, z - c_iz) (periodic wrap in y and z is just a different row address, R2) -- and lane q the copy
+//     of the tile's flag bytes, all completing on the stage's "full" mbarrier (complete_tx).  S stages are
+//     filled ahead; the stage of tile k is refilled (tile k+S) right after the CTA barrier of tile k;
+//   * the x +- 1 shift of 10 of the 19 directions is a shared-memory read at offset +- 1 element; the
+//     periodic wrap in x reads the other end of the same segment when the tile is the whole row, else a 16-byte
+//     halo copy per shifted direction fills the pad in front of / behind the segment;
+//   * results are encoded into a double-buffered output tile and leave with q bulk stores;
+//   * cells with any flag bit set (wall, or next to a wall; lbm_set_flags marks the latter) take the per-cell
+//     path of lbm_kernels.cuh (PullDirWall: neighbour-flag gathers, bounce-back, moving wall) and put their
+//     results into the same output tile; a wall cell re-writes its own unchanged values (both buffers hold the
+//     same values for wall cells: R11 writes both, no step ever changes them).
+// Arithmetic, operation order and codecs are those of lbm_lattice.cuh / lbm_codecs.cuh: the stored results
+// are bit-identical to stream_collide_kernel's and to the oracle's.
+#pragma once
+#include "lbm_kernels.cuh"
+
+namespace lbmk {
+
+struct BulkGeom {
+    int tiles_per_row;     // ceil(nx / TX)
+    int n_tiles;           // tiles_per_row * ny * nz
+};
+
+// ---- PTX wrappers --------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LBM_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LBM_DONE_%=;\n"
+        "bra LBM_WAIT_%=;\n"
+        "LBM_DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+// global -> shared, completes `bytes` on the mbarrier; addresses and size are multiples of 16
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
+                 : "memory");
+}
+// shared -> global, tracked by the issuing thread's bulk async-group
+__device__ __forceinline__ void bulk_s2g(void *dst, unsigned src, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+template <int ID, int COUNT>
+__device__ __forceinline__ void named_bar_sync() {
+    asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(COUNT) : "memory");
+}
+
+// ---- compile-time shape ----------------------------------------------------------------------------
+template <int Q, int F, int NT>
+struct BulkShape {
+    typedef Elem<F> E;
+    static constexpr int ES = E::SIZE;                  // bytes per stored DDF
+    static constexpr int TX = 2 * NT;                   // cells per tile
+    static constexpr int PAD = 16;                      // halo pad in front of and behind every segment
+    static constexpr int ROWB = TX * ES + 2 * PAD;      // one direction of one stage
+    static constexpr int STAGEB = Q * ROWB + TX;        // + the tile's flag bytes
+    static constexpr int OUTROWB = TX * ES;
+    static constexpr int OUTB = Q * OUTROWB;
+    static constexpr int S = ES == 2 ? 3 : 2;           // input stages
+    static constexpr int BAR_OFF = S * STAGEB + 2 * OUTB;
+    static constexpr int SMEM = BAR_OFF + S * 8;
+    static constexpr int HALO_ELEMS = PAD / ES;         // elements in one 16-byte halo copy
+};
+
+// shared-memory access (addresses are "thread base + immediate")
+__device__ __forceinline__ unsigned lds_u32(const char *p) { return *reinterpret_cast<const unsigned *>(p); }
+__device__ __forceinline__ int lds_s16(const char *p) { return (int)*reinterpret_cast<const short *>(p); }
+__device__ __forceinline__ float lds_f32(const char *p) { return *reinterpret_cast<const float *>(p); }
+
+// the two values of direction I for the thread's cells xl, xl+1, from the staged segment.
+//   own  = address of element xl of direction 0's segment; left = element "xl - 1", right = element "xl + 2"
+//   (already wrapped / pointing into the pads); direction I adds the immediate I * ROWB.
+template <int Q, int F, int NT, int I>
+struct PullStaged {
+    typedef BulkShape<Q, F, NT> SH;
+    typedef PairCodec<F> PC;
+    static __device__ __forceinline__ void run(const char *own, const char *left, const char *right, float (&f)[2][Q]) {
+        typedef Lat<Q> L;
+        constexpr int cx = L::c(I, 0);
+        constexpr int o = I * SH::ROWB;
+        if constexpr (SH::ES == 4) {
+            if (cx == 0) {
+                const float2 v = *reinterpret_cast<const float2 *>(own + o);
+                f[0][I] = v.x;
+                f[1][I] = v.y;
+            } else if (cx > 0) {              // sources xl-1, xl
+                f[0][I] = lds_f32(left + o);
+                f[1][I] = lds_f32(own + o);
+            } else {                          // sources xl+1, xl+2
+                f[0][I] = lds_f32(own + o + 4);
+                f[1][I] = lds_f32(right + o);
+            }
+        } else {
+            if (cx == 0) {
+                PC::dec2(lds_u32(own + o), f[0][I], f[1][I]);
+            } else if (cx > 0) {
+                f[0][I] = PC::dec1(lds_s16(left + o));
+                f[1][I] = PC::dec1(lds_s16(own + o));
+            } else {
+                f[0][I] = PC::dec1(lds_s16(own + o + 2));
+                f[1][I] = PC::dec1(lds_s16(right + o));
+            }
+        }
+        PullStaged<Q, F, NT, I + 1>::run(own, left, right, f);
+    }
+};
+template <int Q, int F, int NT>
+struct PullStaged<Q, F, NT, Q> {
+    static __device__ __forceinline__ void run(const char *, const char *, const char *, float (&)[2][Q]) {}
+};
+
+// issue the copies of one tile into one stage: lane i < Q direction i, lane Q the flag bytes (one warp calls this)
+template <int Q, int F, int NT>
+__device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__restrict__ A, const Params &p, int t, int tpr,
+                                                 unsigned stage, unsigned full, int lane, int cx, int cy, int cz) {
+    typedef BulkShape<Q, F, NT> SH;
+    typedef typename Elem<F>::T T;
+    constexpr int ES = SH::ES, TX = SH::TX;
+    constexpr int n_shift = (Q == 9 ? 6 : Q == 19 ? 10 : 18);               // directions with c_x != 0
+    const bool single = tpr == 1;
+    const int row = t / tpr, xt = t - row * tpr;
+    const int z = row / p.ny, y = row - z * p.ny;
+    const int x0 = xt * TX;
+    const int w = min(TX, p.nx - x0);                                       // cells in this tile (multiple of 16)
+    if (lane == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * w * ES + w + (single ? 0 : n_shift * SH::PAD)));
+    __syncwarp();
+    if (lane < Q) {
+        int ys = y - cy, zs = z - cz;                                       // R2: pull source row, periodic
+        ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
+        zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
+        const T *src_row = A + (long long)lane * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+        const unsigned dst = stage + lane * SH::ROWB + SH::PAD;
+        bulk_g2s(dst, src_row + x0, (unsigned)(w * ES), full);
+        if (!single && cx != 0) {
+            if (cx > 0) {                                                   // element x0 - 1: the chunk before x0
+                const int xs = (x0 == 0 ? p.nx : x0) - SH::HALO_ELEMS;
+                bulk_g2s(dst - SH::PAD, src_row + xs, SH::PAD, full);
+            } else {                                                        // element x0 + w: the chunk after the tile
+                const int xs = x0 + w == p.nx ? 0 : x0 + w;
+                bulk_g2s(dst + w * ES, src_row + xs, SH::PAD, full);
+            }
+        }
+    } else if (lane == Q) {
+        const long long own_row = (long long)p.nx * (y + (long long)p.ny * z);
+        bulk_g2s(stage + Q * SH::ROWB, p.flags + own_row + x0, (unsigned)w, full);
+    }
+}
+
+template <int Q, int F, int NT, int MINB, bool FORCE>
+__global__ void __launch_bounds__(NT, MINB)
+stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p,
+                           const BulkGeom g) {
+    typedef BulkShape<Q, F, NT> SH;
+    typedef Elem<F> E;
+    typedef typename E::T T;
+    typedef Lat<Q> L;
+    constexpr int ES = SH::ES, TX = SH::TX, S = SH::S;
+    constexpr int SC = PairCodec<F>::SC;
+    static_assert(Q + 1 <= 32, "one copy-issuing lane per direction + one for the flags");
+    static_assert(SH::STAGEB % 16 == 0 && SH::OUTB % 16 == 0 && SH::ROWB % 16 == 0, "bulk copies need 16-byte alignment");
+
+    extern __shared__ __align__(128) char smem[];
+    const unsigned smem_base = smem_addr(smem);
+    const unsigned bar_full = smem_base + SH::BAR_OFF;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) mbar_init(bar_full + s * 8, 1);          // the issuing warp's arrive.expect_tx
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_async_smem();
+    }
+    __syncthreads();
+
+    const int tpr = g.tiles_per_row;
+    const bool single = tpr == 1;                        // the tile is the whole row: x wraps inside the segment
+    const int stride = gridDim.x;
+
+    // warp 0 moves the data: lane i owns direction i (lane Q the flags)
+    int cx = 0, cy = 0, cz = 0;
+    if (warp == 0) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i)
+            if (i == lane) { cx = L::c(i, 0); cy = L::c(i, 1); cz = L::c(i, 2); }
+#pragma unroll 1
+        for (int s = 0; s < S; ++s) {                                        // prologue: fill every stage
+            const long long t = (long long)blockIdx.x + (long long)s * stride;
+            if (t < g.n_tiles)
+                issue_tile_loads<Q, F, NT>(A, p, (int)t, tpr, smem_base + s * SH::STAGEB, bar_full + s * 8, lane, cx, cy, cz);
+        }
+    }
+
+    const int xl = 2 * tid;
+    int k = 0;
+    for (int t = blockIdx.x; t < g.n_tiles; t += stride, ++k) {
+        const int s = k % S;
+        const unsigned ph = (unsigned)(k / S) & 1u;
+        const int row = t / tpr, xt = t - row * tpr;
+        const int z = row / p.ny, y = row - z * p.ny;
+        const int x0 = xt * TX;
+        const int w = min(TX, p.nx - x0);
+        const bool active = xl < w;
+        const char *stage = smem + s * SH::STAGEB;
+        char *out = smem + S * SH::STAGEB + (k & 1) * SH::OUTB;
+
+        mbar_wait(bar_full + s * 8, ph);
+        unsigned fl = 0;
+        if (active) fl = *reinterpret_cast<const unsigned short *>(stage + Q * SH::ROWB + xl);
+        float f[2][Q];
+        const bool fast = active && fl == 0;
+        if (fast) {
+            const int el = xl - 1 + ((single && xl == 0) ? w : 0);              // element "xl - 1"
+            const int er = xl + 2 - ((single && xl + 2 == w) ? w : 0);          // element "xl + 2"
+            const char *base = stage + SH::PAD;
+            PullStaged<Q, F, NT, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f);
+            collide_bgk<Q, FORCE, SC>(f[0], p);
+            collide_bgk<Q, FORCE, SC>(f[1], p);
+#pragma unroll
+            for (int i = 0; i < Q; ++i) {
+                char *o = out + i * SH::OUTROWB + xl * ES;
+                if constexpr (ES == 4) *reinterpret_cast<float2 *>(o) = make_float2(f[0][i], f[1][i]);
+                else *reinterpret_cast<unsigned *>(o) = PairCodec<F>::enc2(f[0][i], f[1][i]);
+            }
+        } else if (active) {
+            // a wall cell or a wall among the pull sources: cell by cell from global memory (lbm_kernels.cuh)
+            const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
+            const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
+            const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
+            long long rows[3][3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
+#pragma unroll 1
+            for (int j = 0; j < 2; ++j) {
+                const int x = x0 + xl + j;
+                T *o = reinterpret_cast<T *>(out) + xl + j;
+                if ((fl >> (8 * j)) & FLAG_WALL) {                              // not updated
+#pragma unroll
+                    for (int i = 0; i < Q; ++i) o[i * TX] = __ldg(A + (long long)i * p.N + rows[1][1] + x);
+                } else {
+                    const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
+                    float gq[Q];
+                    PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, gq);
+                    collide_bgk<Q, FORCE, 0>(gq, p);
+#pragma unroll
+                    for (int i = 0; i < Q; ++i) E::st1(o + i * TX, gq[i]);
+                }
+            }
+        }
+        fence_async_smem();                                                     // generic-proxy writes -> bulk store
+        if (warp == 0 && lane < Q) bulk_wait_read0();                           // tile k-1's stores have left smem
+        __syncthreads();            // everyone has read stage s and written `out`; the other out buffer is free
+        if (warp == 0) {
+            if (lane < Q) {
+                T *dst = B + (long long)lane * p.N + (long long)p.nx * (y + (long long)p.ny * z) + x0;
+                bulk_s2g(dst, smem_addr(out) + lane * SH::OUTROWB, (unsigned)(w * ES));
+                bulk_commit();
+            }
+            const long long tn = (long long)t + (long long)S * stride;          // refill the stage just consumed
+            if (tn < g.n_tiles)
+                issue_tile_loads<Q, F, NT>(A, p, (int)tn, tpr, smem_base + s * SH::STAGEB, bar_full + s * 8, lane, cx, cy, cz);
+        }
+    }
+    if (warp == 0 && lane < Q) bulk_wait0();
+}
+
+}  // namespace lbmk

@@ -150,4 +150,69 @@ struct Codec<F_P16_2C> {
     }
 };
 
+// ---- codecs on pairs: two 16-bit codes in one 32-bit word (low half = the lower x) ----------------------
+// Used by the shared-memory-staged kernel (lbm_bulk.cuh), which handles two neighbouring cells per thread.
+//   SC        the decoded values are 2^SC times the DDFs and enc2 expects 2^SC times the DDFs: FP16S leaves its
+//             2^15 scaling to the collision (collide_bgk<.., SC>), which folds it into operations it executes
+//             anyway -- decode is one HADD2.F32, encode half an F2FP.PACK_AB per value;
+//   dec1(c)   c = one code SIGN-EXTENDED to 32 bits (ld.shared.s16);
+//   dec2(w)   both codes of a word;  enc2(a, b) packs the codes of a (low) and b (high).
+// Every function returns bit for bit what Codec<F>::dec / enc return (times 2^SC).
+template <int F>
+struct PairCodec {
+    static constexpr int SC = 0;
+    static __device__ __forceinline__ float dec1(int c) { return Codec<F>::dec((unsigned)c & 0xFFFFu); }
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        a = Codec<F>::dec(w & 0xFFFFu);
+        b = Codec<F>::dec(w >> 16);
+    }
+    static __device__ __forceinline__ unsigned enc2(float a, float b) { return Codec<F>::enc(a) | (Codec<F>::enc(b) << 16); }
+};
+
+template <int SCALE>
+struct PairHalf {
+    static constexpr int SC = SCALE;
+    static __device__ __forceinline__ float dec1(int c) { return __half2float(__ushort_as_half((unsigned short)c)); }
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        const float2 v = __half22float2(*reinterpret_cast<const __half2 *>(&w));
+        a = v.x;
+        b = v.y;
+    }
+    static __device__ __forceinline__ unsigned enc2(float a, float b) {
+        const __half2 h = __floats2half2_rn(a, b);          // one F2FP.F16.F32.PACK_AB, round-to-nearest-even
+        return *reinterpret_cast<const unsigned *>(&h);
+    }
+};
+template <>
+struct PairCodec<F_FP16> : PairHalf<0> {};
+template <>
+struct PairCodec<F_FP16S> : PairHalf<15> {};
+
+// FP16C: the sign-extended code shifted left by 12 has the sign in bits 31..27 and the magnitude in bits 26..12;
+// one AND leaves sign | magnitude, the multiply by 2^112 does exponent re-bias and denormals (Codec<F_FP16C>).
+// Encode: clamp |x| to the largest value (NaN -> largest, as Codec does), fmul.rz by 2^-112, add half an ulp;
+// the magnitude code then sits in bits 26..12: shifted left by 4 it is the upper half-word, and one PRMT packs
+// two of them; a second PRMT gathers the two sign bytes.
+template <>
+struct PairCodec<F_FP16C> {
+    static constexpr int SC = 0;
+    static __device__ __forceinline__ float bits2f(unsigned t) {
+        return __fmul_rn(__uint_as_float(t & 0x87FFF000u), __uint_as_float(0x77800000u));   // * 2^112, exact
+    }
+    static __device__ __forceinline__ float dec1(int c) { return bits2f((unsigned)c << 12); }
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        a = bits2f((unsigned)((int)(w << 16) >> 4));
+        b = bits2f((unsigned)((int)w >> 4));
+    }
+    static __device__ __forceinline__ unsigned mag4(float x) {      // magnitude code in bits 30..16
+        const float y = __fmul_rz(fminf(fabsf(x), __uint_as_float(0x3FFFF000u) /* 2 - 2^-11 */), __uint_as_float(0x07800000u));
+        return (__float_as_uint(y) + 0x800u) << 4;
+    }
+    static __device__ __forceinline__ unsigned enc2(float a, float b) {
+        const unsigned mags = __byte_perm(mag4(a), mag4(b), 0x7632);
+        const unsigned signs = __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x7632);
+        return (mags & 0x7FFF7FFFu) | (signs & 0x80008000u);
+    }
+};
+
 }  // namespace lbmk

@@ -8,12 +8,16 @@
 
 namespace lbmk {
 
+constexpr int VARIANT_BULK = 16;      // LBM_VARIANT_BULK of include/lbm.h
+
 struct UnitOps {
-    // stream_collide: V cells per thread (1, 2 or 4; nx % V == 0), force = Guo term compiled in
+    // stream_collide: V = cells per thread (1, 2 or 4; nx % V == 0) of the per-thread kernel, or VARIANT_BULK
+    // = the shared-memory-staged kernel (nx % 16 == 0); force = Guo term compiled in
     cudaError_t (*stream_collide)(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st);
     cudaError_t (*init)(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st);
     cudaError_t (*read)(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st);
     const char *(*name)(int V, int coll, bool force);
+    int (*bulk_tile_cells)();     // cells per tile of the staged kernel
 };
 
 const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)
@@ -21,6 +25,7 @@ const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compile
 // lbm_aux.cu
 cudaError_t launch_mark_near(int q, const unsigned char *in, unsigned char *out, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t launch_codec(int fmt, bool encode, const void *in, void *out, long long count, cudaStream_t st);
+cudaError_t launch_pair_selftest(int fmt, unsigned long long *mismatches_dev, cudaStream_t st);
 
 void count_launch(long long n = 1);
 

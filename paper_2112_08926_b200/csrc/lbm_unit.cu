@@ -2,6 +2,7 @@
 // lbm_kernels.cuh.  Compiled once per pair with -DLBM_Q=<9|19|27> -DLBM_F=<0..6> (see build.py).
 #include "lbm_internal.h"
 #include "lbm_kernels.cuh"
+#include "lbm_bulk.cuh"
 
 #ifndef LBM_Q
 #error "compile with -DLBM_Q=<velocity set> -DLBM_F=<format>"
@@ -32,8 +33,42 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
     return cudaGetLastError();
 }
 
+
+// ---- the shared-memory-staged variant (lbm_bulk.cuh) ------------------------------------------------
+// consumer threads per CTA and CTAs per SM, by velocity set: shared memory per CTA is
+// S*(Q*(2*NT*ES+32)+2*NT) + 2*Q*2*NT*ES bytes
+constexpr int BULK_NT = Q == 27 ? 128 : (Elem<F>::SIZE == 4 ? 128 : 256);
+constexpr int BULK_MINB = Q == 9 ? 3 : Q == 19 ? 2 : 3;
+
+template <bool FORCE>
+cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st) {
+    typedef BulkShape<Q, F, BULK_NT> SH;
+    auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, BULK_MINB, FORCE>;
+    static int ctas = 0;                      // resident CTAs on the device, resolved once per instantiation
+    if (ctas == 0) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SH::SMEM);
+        if (e != cudaSuccess) return e;
+        int dev = 0, sms = 0, per_sm = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BULK_NT, SH::SMEM)) != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        ctas = sms * per_sm;
+    }
+    BulkGeom g;
+    g.tiles_per_row = (p.nx + SH::TX - 1) / SH::TX;
+    const long long tiles = (long long)g.tiles_per_row * p.ny * p.nz;
+    if (p.nx % 16 != 0 || tiles > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
+    g.n_tiles = (int)tiles;
+    const int grid = (int)(tiles < ctas ? tiles : ctas);
+    kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g);
+    count_launch();
+    return cudaGetLastError();
+}
+
 cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
     (void)coll;
+    if (V == VARIANT_BULK) return force ? launch_bulk<true>(A, B, p, st) : launch_bulk<false>(A, B, p, st);
     switch (V * 2 + (force ? 1 : 0)) {
         case 2: return launch_sc<1, false>(A, B, p, st);
         case 3: return launch_sc<1, true>(A, B, p, st);
@@ -66,19 +101,23 @@ cudaError_t read(const void *A, const Params &p, bool force, float *rho, float *
 
 const char *name(int V, int coll, bool force) {
     (void)coll;
-    static const char *names[3][2] = {
+    static const char *names[4][2] = {
         {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=0>",
          "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=1>"},
         {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=0>",
          "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=1>"},
         {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=0>",
-         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=1>"}};
-    return names[V == 1 ? 0 : V == 2 ? 1 : 2][force ? 1 : 0];
+         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=1>"},
+        {"stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0>",
+         "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1>"}};
+    return names[V == 1 ? 0 : V == 2 ? 1 : V == 4 ? 2 : 3][force ? 1 : 0];
 }
+
+int bulk_tile_cells() { return 2 * BULK_NT; }
 
 }  // namespace
 
 extern const UnitOps LBM_UNIT_SYMBOL;
-const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name};
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells};
 
 }  // namespace lbmk

@@ -71,3 +71,10 @@ def test_codec_edge_cases():
     assert lbm.codec_encode("FP16C", np.zeros(0, np.float32)).size == 0
     with pytest.raises(lbm.LbmError):
         lbm.codec_encode("FP32", np.zeros(4, np.float32))
+
+
+@pytest.mark.parametrize("name", [n for n in FORMATS if n != "FP32"])
+def test_pair_codecs_equal_scalar_codecs_exhaustively(name):
+    """The staged kernel's converters (PairCodec) vs the scalar ones (compared with the oracle above): all 65 536
+    codes and all 2^32 FP32 bit patterns, on the device."""
+    assert lbm.codec_pair_selftest(name) == 0

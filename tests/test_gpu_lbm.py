@@ -20,9 +20,9 @@ ALL_FORMATS = list(FORMATS)
 TOL = {name: (1e-6 if name == "FP32" else 1e-3) for name in ALL_FORMATS}
 
 
-def run_pair(w, name, steps, cells_per_thread=0):
+def run_pair(w, name, steps, cells_per_thread=0, variant=0):
     osim = oracle.from_workload(w, FORMATS[name])
-    gsim = lbm.from_workload(w, name, cells_per_thread=cells_per_thread)
+    gsim = lbm.from_workload(w, name, cells_per_thread=cells_per_thread, variant=variant)
     osim.step(steps)
     gsim.step(steps)
     return osim, gsim
@@ -144,3 +144,51 @@ def test_mass_conservation_fp32():
     gsim.step(200)
     m1 = sum(gsim.read_ddf(i).astype(np.float64).sum() for i in range(19))
     assert abs(m1 - m0) / w.n_cells < 1e-6
+
+
+# ---- the shared-memory-staged kernel (lbm_bulk.cuh): same results, bit for bit ------------------------
+# shapes: one tile per row (x wraps inside the segment), several tiles per row with a ragged last tile (halo
+# copies, wrap at the row ends), the smallest legal row (16 cells), 2-D
+BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16, 4, 5)), (19, (512, 2, 1)),
+               (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1))]
+
+
+@pytest.mark.parametrize("q,shape", BULK_SHAPES)
+@pytest.mark.parametrize("name", ALL_FORMATS)
+def test_bulk_variant_periodic(q, shape, name):
+    w = wl.perturbed_equilibrium(*shape, seed=21, velset=q)
+    osim, gsim = run_pair(w, name, 12, variant=lbm.VARIANT_BULK)
+    assert "bulk" in gsim.kernel_name
+    assert_parity(osim, gsim, name)
+
+
+@pytest.mark.parametrize("q,shape", [(19, (48, 7, 5)), (19, (544, 3, 3)), (27, (32, 6, 5)), (9, (64, 11, 1))])
+@pytest.mark.parametrize("name", ALL_FORMATS)
+def test_bulk_variant_walls_moving_walls_force(q, shape, name):
+    w = wl.perturbed_equilibrium(*shape, seed=23, velset=q, tau=0.7)
+    w = wl.random_walls(w, 0.12, seed=29, moving_fraction=0.5)
+    w.force = (1e-5, -2e-5, 0.0 if q == 9 else 3e-5)
+    osim, gsim = run_pair(w, name, 25, variant=lbm.VARIANT_BULK)
+    assert "bulk" in gsim.kernel_name
+    assert_parity(osim, gsim, name)
+
+
+@pytest.mark.parametrize("name", ["FP16S", "FP16C", "P16_0S"])
+def test_bulk_variant_taylor_green_and_cavity(name):
+    w = wl.taylor_green_3d(32)
+    osim, gsim = run_pair(w, name, 200, variant=lbm.VARIANT_BULK)
+    assert_parity(osim, gsim, name)
+    w = wl.lid_driven_cavity(32, tau=0.5384)
+    osim, gsim = run_pair(w, name, 300, variant=lbm.VARIANT_BULK)
+    assert_parity(osim, gsim, name)
+
+
+def test_automatic_variant_choice():
+    w = wl.perturbed_equilibrium(256, 2, 2, seed=2)
+    g16 = lbm.from_workload(w, "FP16S")
+    g32 = lbm.from_workload(w, "FP32")
+    assert "bulk" in g16.kernel_name and "bulk" not in g32.kernel_name
+    w = wl.perturbed_equilibrium(36, 2, 2, seed=2)          # rows not 16-cell aligned: per-thread kernel
+    assert "bulk" not in lbm.from_workload(w, "FP16S").kernel_name
+    with pytest.raises(lbm.LbmError):
+        lbm.from_workload(w, "FP16S", variant=lbm.VARIANT_BULK)
