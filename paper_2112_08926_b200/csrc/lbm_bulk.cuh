@@ -11,10 +11,11 @@
 // Shape of the kernel
 //   * persistent CTAs (grid = SMs x resident CTAs), tiles handed out round-robin; a tile is up to TX = 2*NT
 //     consecutive cells of one row (y, z); NT consumer threads handle two neighbouring cells each;
-//   * warp 0 moves the data: lane i < q issues the copy of direction i -- TX elements of source row
-//     (y - c_iy, z - c_iz) (periodic wrap in y and z is just a different row address, R2) -- and lane q the copy
-//     of the tile's flag bytes, all completing on the stage's "full" mbarrier (complete_tx).  S stages are
-//     filled ahead; the stage of tile k is refilled (tile k+S) right after the CTA barrier of tile k;
+//   * every warp moves a share of the data (one lane issues; the bulk-copy instruction is warp-uniform): warp v
+//     the directions v, v+NW, ... -- the copy of direction i is TX elements of source row (y - c_iy, z - c_iz)
+//     (periodic wrap in y and z is just a different row address, R2) -- plus one copy of the tile's flag bytes,
+//     all completing on the stage's "full" mbarrier (complete_tx).  S stages are filled ahead; the stage of
+//     tile k is refilled (tile k+S) right after the CTA barrier of tile k;
 //   * the x +- 1 shift of 10 of the 19 directions is a shared-memory read at offset +- 1 element; the
 //     periodic wrap in x reads the other end of the same segment when the tile is the whole row, else a 16-byte
 //     halo copy per shifted direction fills the pad in front of / behind the segment;
@@ -30,10 +31,35 @@
 
 namespace lbmk {
 
+// exact n / d for 0 <= n < 2^31 as (n * M) >> sh, M = floor(2^sh / d) + 1, sh = 31 + ceil(log2 d)
+struct FastDiv {
+    unsigned M;
+    int sh;
+    __host__ static FastDiv make(int d) {
+        FastDiv f;
+        int s = 0;
+        while ((1LL << s) < d) ++s;
+        f.sh = 31 + s;
+        f.M = (unsigned)((1ULL << f.sh) / (unsigned long long)d + 1ULL);
+        return f;
+    }
+    __device__ __forceinline__ int div(int n) const { return (int)(((unsigned long long)(unsigned)n * M) >> sh); }
+};
+
 struct BulkGeom {
     int tiles_per_row;     // ceil(nx / TX)
-    int n_tiles;           // tiles_per_row * ny * nz
+    int n_tiles;           // tiles_per_row * ny * nz  (< 2^31)
+    FastDiv by_tpr, by_ny;
 };
+
+// c_i of the library's numbering for a run-time direction index (copy issue only; the collision uses Lat<Q>)
+static __constant__ signed char c27_table[27][3] = {{0, 0, 0},
+                                             {1, 0, 0},   {-1, 0, 0},  {0, 1, 0},   {0, -1, 0},  {0, 0, 1},   {0, 0, -1},
+                                             {1, 1, 0},   {-1, -1, 0}, {1, 0, 1},   {-1, 0, -1}, {0, 1, 1},   {0, -1, -1},
+                                             {1, -1, 0},  {-1, 1, 0},  {1, 0, -1},  {-1, 0, 1},  {0, 1, -1},  {0, -1, 1},
+                                             {1, 1, 1},   {-1, -1, -1}, {1, 1, -1}, {-1, -1, 1}, {1, -1, 1},  {-1, 1, -1},
+                                             {-1, 1, 1},  {1, -1, -1}};
+static __constant__ signed char d2q9_members[9] = {0, 1, 2, 3, 4, 7, 8, 13, 14};
 
 // ---- PTX wrappers --------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -142,40 +168,57 @@ struct PullStaged<Q, F, NT, Q> {
     static __device__ __forceinline__ void run(const char *, const char *, const char *, float (&)[2][Q]) {}
 };
 
-// issue the copies of one tile into one stage: lane i < Q direction i, lane Q the flag bytes (one warp calls this)
+struct TileCoord {
+    int y, z, x0, w;       // row, first cell and number of cells (multiple of 16) of a tile
+};
+template <int TX>
+__device__ __forceinline__ TileCoord tile_coord(int t, const BulkGeom &g, const Params &p) {
+    TileCoord c;
+    const int row = g.by_tpr.div(t), xt = t - row * g.tiles_per_row;
+    c.z = g.by_ny.div(row);
+    c.y = row - c.z * p.ny;
+    c.x0 = xt * TX;
+    c.w = min(TX, p.nx - c.x0);
+    return c;
+}
+
+// The copies of one tile into one stage.  Every warp issues the directions i = warp, warp + NW, ... (i = Q: the
+// flag bytes): the index is warp-uniform, one lane issues.
 template <int Q, int F, int NT>
-__device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__restrict__ A, const Params &p, int t, int tpr,
-                                                 unsigned stage, unsigned full, int lane, int cx, int cy, int cz) {
+__device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__restrict__ A, const Params &p, const BulkGeom &g,
+                                                 int t, unsigned stage, unsigned full, int warp, int lane) {
     typedef BulkShape<Q, F, NT> SH;
     typedef typename Elem<F>::T T;
-    constexpr int ES = SH::ES, TX = SH::TX;
+    constexpr int ES = SH::ES, TX = SH::TX, NW = NT / 32;
     constexpr int n_shift = (Q == 9 ? 6 : Q == 19 ? 10 : 18);               // directions with c_x != 0
-    const bool single = tpr == 1;
-    const int row = t / tpr, xt = t - row * tpr;
-    const int z = row / p.ny, y = row - z * p.ny;
-    const int x0 = xt * TX;
-    const int w = min(TX, p.nx - x0);                                       // cells in this tile (multiple of 16)
-    if (lane == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * w * ES + w + (single ? 0 : n_shift * SH::PAD)));
-    __syncwarp();
-    if (lane < Q) {
-        int ys = y - cy, zs = z - cz;                                       // R2: pull source row, periodic
+    const bool single = g.tiles_per_row == 1;
+    const TileCoord c = tile_coord<TX>(t, g, p);
+    if (lane != 0) return;
+    if (warp == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * c.w * ES + c.w + (single ? 0 : n_shift * SH::PAD)));
+#pragma unroll 1
+    for (int i = warp; i <= Q; i += NW) {
+        if (i == Q) {
+            const long long own_row = (long long)p.nx * (c.y + (long long)p.ny * c.z);
+            bulk_g2s(stage + Q * SH::ROWB, p.flags + own_row + c.x0, (unsigned)c.w, full);
+            break;
+        }
+        const int m = Q == 9 ? d2q9_members[i] : i;
+        const int cx = c27_table[m][0], cy = c27_table[m][1], cz = c27_table[m][2];
+        int ys = c.y - cy, zs = c.z - cz;                                   // R2: pull source row, periodic
         ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
         zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
-        const T *src_row = A + (long long)lane * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
-        const unsigned dst = stage + lane * SH::ROWB + SH::PAD;
-        bulk_g2s(dst, src_row + x0, (unsigned)(w * ES), full);
+        const T *src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+        const unsigned dst = stage + i * SH::ROWB + SH::PAD;
+        bulk_g2s(dst, src_row + c.x0, (unsigned)(c.w * ES), full);
         if (!single && cx != 0) {
             if (cx > 0) {                                                   // element x0 - 1: the chunk before x0
-                const int xs = (x0 == 0 ? p.nx : x0) - SH::HALO_ELEMS;
+                const int xs = (c.x0 == 0 ? p.nx : c.x0) - SH::HALO_ELEMS;
                 bulk_g2s(dst - SH::PAD, src_row + xs, SH::PAD, full);
             } else {                                                        // element x0 + w: the chunk after the tile
-                const int xs = x0 + w == p.nx ? 0 : x0 + w;
-                bulk_g2s(dst + w * ES, src_row + xs, SH::PAD, full);
+                const int xs = c.x0 + c.w == p.nx ? 0 : c.x0 + c.w;
+                bulk_g2s(dst + c.w * ES, src_row + xs, SH::PAD, full);
             }
         }
-    } else if (lane == Q) {
-        const long long own_row = (long long)p.nx * (y + (long long)p.ny * z);
-        bulk_g2s(stage + Q * SH::ROWB, p.flags + own_row + x0, (unsigned)w, full);
     }
 }
 
@@ -186,10 +229,8 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
     typedef BulkShape<Q, F, NT> SH;
     typedef Elem<F> E;
     typedef typename E::T T;
-    typedef Lat<Q> L;
-    constexpr int ES = SH::ES, TX = SH::TX, S = SH::S;
+    constexpr int ES = SH::ES, TX = SH::TX, S = SH::S, NW = NT / 32;
     constexpr int SC = PairCodec<F>::SC;
-    static_assert(Q + 1 <= 32, "one copy-issuing lane per direction + one for the flags");
     static_assert(SH::STAGEB % 16 == 0 && SH::OUTB % 16 == 0 && SH::ROWB % 16 == 0, "bulk copies need 16-byte alignment");
 
     extern __shared__ __align__(128) char smem[];
@@ -198,28 +239,19 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     if (tid == 0) {
-        for (int s = 0; s < S; ++s) mbar_init(bar_full + s * 8, 1);          // the issuing warp's arrive.expect_tx
+        for (int s = 0; s < S; ++s) mbar_init(bar_full + s * 8, 1);          // warp 0's arrive.expect_tx
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_async_smem();
     }
     __syncthreads();
 
-    const int tpr = g.tiles_per_row;
-    const bool single = tpr == 1;                        // the tile is the whole row: x wraps inside the segment
+    const bool single = g.tiles_per_row == 1;            // the tile is the whole row: x wraps inside the segment
     const int stride = gridDim.x;
 
-    // warp 0 moves the data: lane i owns direction i (lane Q the flags)
-    int cx = 0, cy = 0, cz = 0;
-    if (warp == 0) {
-#pragma unroll
-        for (int i = 0; i < Q; ++i)
-            if (i == lane) { cx = L::c(i, 0); cy = L::c(i, 1); cz = L::c(i, 2); }
 #pragma unroll 1
-        for (int s = 0; s < S; ++s) {                                        // prologue: fill every stage
-            const long long t = (long long)blockIdx.x + (long long)s * stride;
-            if (t < g.n_tiles)
-                issue_tile_loads<Q, F, NT>(A, p, (int)t, tpr, smem_base + s * SH::STAGEB, bar_full + s * 8, lane, cx, cy, cz);
-        }
+    for (int s = 0; s < S; ++s) {                                            // prologue: fill every stage
+        const long long t = (long long)blockIdx.x + (long long)s * stride;
+        if (t < g.n_tiles) issue_tile_loads<Q, F, NT>(A, p, g, (int)t, smem_base + s * SH::STAGEB, bar_full + s * 8, warp, lane);
     }
 
     const int xl = 2 * tid;
@@ -227,10 +259,8 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
     for (int t = blockIdx.x; t < g.n_tiles; t += stride, ++k) {
         const int s = k % S;
         const unsigned ph = (unsigned)(k / S) & 1u;
-        const int row = t / tpr, xt = t - row * tpr;
-        const int z = row / p.ny, y = row - z * p.ny;
-        const int x0 = xt * TX;
-        const int w = min(TX, p.nx - x0);
+        const TileCoord c = tile_coord<TX>(t, g, p);
+        const int y = c.y, z = c.z, x0 = c.x0, w = c.w;
         const bool active = xl < w;
         const char *stage = smem + s * SH::STAGEB;
         char *out = smem + S * SH::STAGEB + (k & 1) * SH::OUTB;
@@ -281,20 +311,19 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             }
         }
         fence_async_smem();                                                     // generic-proxy writes -> bulk store
-        if (warp == 0 && lane < Q) bulk_wait_read0();                           // tile k-1's stores have left smem
+        if (lane == 0) bulk_wait_read0();                                       // this warp's stores of tile k-1 have left smem
         __syncthreads();            // everyone has read stage s and written `out`; the other out buffer is free
-        if (warp == 0) {
-            if (lane < Q) {
-                T *dst = B + (long long)lane * p.N + (long long)p.nx * (y + (long long)p.ny * z) + x0;
-                bulk_s2g(dst, smem_addr(out) + lane * SH::OUTROWB, (unsigned)(w * ES));
-                bulk_commit();
-            }
-            const long long tn = (long long)t + (long long)S * stride;          // refill the stage just consumed
-            if (tn < g.n_tiles)
-                issue_tile_loads<Q, F, NT>(A, p, (int)tn, tpr, smem_base + s * SH::STAGEB, bar_full + s * 8, lane, cx, cy, cz);
+        if (lane == 0) {
+            const long long own = (long long)p.nx * (y + (long long)p.ny * z) + x0;
+#pragma unroll 1
+            for (int i = warp; i < Q; i += NW)
+                bulk_s2g(B + (long long)i * p.N + own, smem_addr(out) + i * SH::OUTROWB, (unsigned)(w * ES));
+            bulk_commit();
         }
+        const long long tn = (long long)t + (long long)S * stride;              // refill the stage just consumed
+        if (tn < g.n_tiles) issue_tile_loads<Q, F, NT>(A, p, g, (int)tn, smem_base + s * SH::STAGEB, bar_full + s * 8, warp, lane);
     }
-    if (warp == 0 && lane < Q) bulk_wait0();
+    if (lane == 0) bulk_wait0();
 }
 
 }  // namespace lbmk

@@ -60,6 +60,8 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
     const long long tiles = (long long)g.tiles_per_row * p.ny * p.nz;
     if (p.nx % 16 != 0 || tiles > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
     g.n_tiles = (int)tiles;
+    g.by_tpr = FastDiv::make(g.tiles_per_row);
+    g.by_ny = FastDiv::make(p.ny);
     const int grid = (int)(tiles < ctas ? tiles : ctas);
     kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g);
     count_launch();
