@@ -50,6 +50,7 @@ struct BulkGeom {
     int tiles_per_row;     // ceil(nx / TX)
     int n_tiles;           // tiles_per_row * ny * nz  (< 2^31)
     FastDiv by_tpr, by_ny;
+    long long src_off[27]; // i*N - nx*(c_iy + ny*c_iz): source row of direction i relative to the own row, no wrap
 };
 
 // c_i of the library's numbering for a run-time direction index (copy issue only; the collision uses Lat<Q>)
@@ -195,19 +196,26 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     const TileCoord c = tile_coord<TX>(t, g, p);
     if (lane != 0) return;
     if (warp == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * c.w * ES + c.w + (single ? 0 : n_shift * SH::PAD)));
+    const long long own = (long long)p.nx * (c.y + (long long)p.ny * c.z);
+    // rows on a y or z face of the box pull some directions from the opposite face (R2): rare, general path
+    const bool face = c.y == 0 || c.y == p.ny - 1 || c.z == 0 || c.z == p.nz - 1;
 #pragma unroll 1
     for (int i = warp; i <= Q; i += NW) {
         if (i == Q) {
-            const long long own_row = (long long)p.nx * (c.y + (long long)p.ny * c.z);
-            bulk_g2s(stage + Q * SH::ROWB, p.flags + own_row + c.x0, (unsigned)c.w, full);
+            bulk_g2s(stage + Q * SH::ROWB, p.flags + own + c.x0, (unsigned)c.w, full);
             break;
         }
         const int m = Q == 9 ? d2q9_members[i] : i;
-        const int cx = c27_table[m][0], cy = c27_table[m][1], cz = c27_table[m][2];
-        int ys = c.y - cy, zs = c.z - cz;                                   // R2: pull source row, periodic
-        ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
-        zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
-        const T *src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+        const int cx = c27_table[m][0];
+        const T *src_row;
+        if (!face) {
+            src_row = A + own + g.src_off[i];
+        } else {
+            int ys = c.y - c27_table[m][1], zs = c.z - c27_table[m][2];
+            ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
+            zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
+            src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+        }
         const unsigned dst = stage + i * SH::ROWB + SH::PAD;
         bulk_g2s(dst, src_row + c.x0, (unsigned)(c.w * ES), full);
         if (!single && cx != 0) {
@@ -236,7 +244,8 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
     extern __shared__ __align__(128) char smem[];
     const unsigned smem_base = smem_addr(smem);
     const unsigned bar_full = smem_base + SH::BAR_OFF;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);                  // warp-uniform by construction
 
     if (tid == 0) {
         for (int s = 0; s < S; ++s) mbar_init(bar_full + s * 8, 1);          // warp 0's arrive.expect_tx

@@ -62,6 +62,8 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
     g.n_tiles = (int)tiles;
     g.by_tpr = FastDiv::make(g.tiles_per_row);
     g.by_ny = FastDiv::make(p.ny);
+    for (int i = 0; i < 27; ++i)
+        g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
     const int grid = (int)(tiles < ctas ? tiles : ctas);
     kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g);
     count_launch();
