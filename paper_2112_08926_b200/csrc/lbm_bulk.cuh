@@ -9,21 +9,24 @@
 // memory every address is "thread base + compile-time immediate".
 //
 // Shape of the kernel
-//   * persistent CTAs (grid = SMs x resident CTAs), tiles handed out round-robin; a tile is up to TX = 2*NT
-//     consecutive cells of one row (y, z); NT consumer threads handle two neighbouring cells each;
-//   * every warp moves a share of the data (one lane issues; the bulk-copy instruction is warp-uniform): warp v
-//     the directions v, v+NW, ... -- the copy of direction i is TX elements of source row (y - c_iy, z - c_iz)
+//   * persistent CTAs (grid = SMs x resident CTAs), tiles handed out round-robin.  A tile is up to TX = 2*NT
+//     consecutive cells of one row (y, z); when a row is a single tile (nx <= TX) a tile is up to RMAX
+//     consecutive rows of one z-plane: in the SoA layout they are ONE contiguous segment per direction, so the
+//     number of copies per cell and all per-tile bookkeeping halve.  NT threads, two neighbouring cells each,
+//     row after row;
+//   * every warp issues a share of the copies (one lane issues; the bulk-copy instruction is warp-uniform): warp v
+//     the directions v, v+NW, ... -- the copy of direction i is the segment of source row (y - c_iy, z - c_iz)
 //     (periodic wrap in y and z is just a different row address, R2) -- plus one copy of the tile's flag bytes,
-//     all completing on the stage's "full" mbarrier (complete_tx).  S stages are filled ahead; the stage of
-//     tile k is refilled (tile k+S) right after the CTA barrier of tile k;
+//     all completing on the stage's "full" mbarrier (complete_tx).  S stages are filled ahead.  A warp that has
+//     its values in registers arrives on the stage's "empty" mbarrier; before issuing its share of the refill
+//     (tile k+S) a warp waits for that barrier -- there is no CTA-wide barrier in the loop;
 //   * the x +- 1 shift of 10 of the 19 directions is a shared-memory read at offset +- 1 element; the
-//     periodic wrap in x reads the other end of the same segment when the tile is the whole row, else a 16-byte
+//     periodic wrap in x reads the other end of the same row when the tile spans the row, else a 16-byte
 //     halo copy per shifted direction fills the pad in front of / behind the segment;
-//   * results are encoded into a double-buffered output tile and leave with q bulk stores;
+//   * results are encoded in registers and stored directly (one aligned 32/64-bit store per direction and cell
+//     pair, 128/256 contiguous bytes per warp): stores need no latency hiding, so they need no staging;
 //   * cells with any flag bit set (wall, or next to a wall; lbm_set_flags marks the latter) take the per-cell
-//     path of lbm_kernels.cuh (PullDirWall: neighbour-flag gathers, bounce-back, moving wall) and put their
-//     results into the same output tile; a wall cell re-writes its own unchanged values (both buffers hold the
-//     same values for wall cells: R11 writes both, no step ever changes them).
+//     path of lbm_kernels.cuh (PullDirWall: neighbour-flag gathers, bounce-back, moving wall).
 // Arithmetic, operation order and codecs are those of lbm_lattice.cuh / lbm_codecs.cuh: the stored results
 // are bit-identical to stream_collide_kernel's and to the oracle's.
 #pragma once
@@ -48,8 +51,10 @@ struct FastDiv {
 
 struct BulkGeom {
     int tiles_per_row;     // ceil(nx / TX)
-    int n_tiles;           // tiles_per_row * ny * nz  (< 2^31)
-    FastDiv by_tpr, by_ny;
+    int rows_per_tile;     // RMAX if tiles_per_row == 1, else 1
+    int ytiles;            // ceil(ny / rows_per_tile)
+    int n_tiles;           // tiles_per_row * ytiles * nz  (< 2^31)
+    FastDiv by_tpr, by_ytiles;
     long long src_off[27]; // i*N - nx*(c_iy + ny*c_iz): source row of direction i relative to the own row, no wrap
 };
 
@@ -110,16 +115,19 @@ template <int Q, int F, int NT>
 struct BulkShape {
     typedef Elem<F> E;
     static constexpr int ES = E::SIZE;                  // bytes per stored DDF
-    static constexpr int TX = 2 * NT;                   // cells per tile
+    static constexpr int TX = 2 * NT;                   // cells per tile row
     static constexpr int PAD = 16;                      // halo pad in front of and behind every segment
-    static constexpr int ROWB = TX * ES + 2 * PAD;      // one direction of one stage
-    static constexpr int STAGEB = Q * ROWB + TX;        // + the tile's flag bytes
-    static constexpr int OUTROWB = TX * ES;
-    static constexpr int OUTB = Q * OUTROWB;
-    static constexpr int S = ES == 2 ? 3 : 2;           // input stages
-    static constexpr int BAR_OFF = S * STAGEB + 2 * OUTB;
-    static constexpr int SMEM = BAR_OFF + S * 8;
-    static constexpr int HALO_ELEMS = PAD / ES;         // elements in one 16-byte halo copy
+    static constexpr int MAXB = (227 * 1024 - 2048) / 2;                    // two CTAs per SM
+    static constexpr int row_stage(int r) { return Q * (r * TX * ES + 2 * PAD) + r * TX; }
+    static constexpr int RMAX = 2 * row_stage(2) <= MAXB ? 2 : 1;           // rows per tile (single-tile rows only)
+    static constexpr int ROWB = RMAX * TX * ES + 2 * PAD;                   // one direction of one stage
+    static constexpr int STAGEB = row_stage(RMAX);                          // + the tile's flag bytes
+    static constexpr int S = 3 * STAGEB <= MAXB ? 3 : 2;                    // input stages
+    static constexpr int BAR_OFF = S * STAGEB;
+    static constexpr int SMEM = BAR_OFF + 2 * S * 8;                        // full[S], empty[S]
+    static constexpr int HALO_ELEMS = PAD / ES;                             // elements in one 16-byte halo copy
+    static_assert(2 * STAGEB <= MAXB, "two stages of two CTAs must fit one SM");
+    static_assert(STAGEB % 16 == 0 && ROWB % 16 == 0, "bulk copies need 16-byte alignment");
 };
 
 // shared-memory access (addresses are "thread base + immediate")
@@ -170,21 +178,22 @@ struct PullStaged<Q, F, NT, Q> {
 };
 
 struct TileCoord {
-    int y, z, x0, w;       // row, first cell and number of cells (multiple of 16) of a tile
+    int y, z, x0, w, rows;   // first row, plane, first cell, cells per row (multiple of 16), rows of a tile
 };
 template <int TX>
 __device__ __forceinline__ TileCoord tile_coord(int t, const BulkGeom &g, const Params &p) {
     TileCoord c;
-    const int row = g.by_tpr.div(t), xt = t - row * g.tiles_per_row;
-    c.z = g.by_ny.div(row);
-    c.y = row - c.z * p.ny;
+    const int rt = g.by_tpr.div(t), xt = t - rt * g.tiles_per_row;
+    c.z = g.by_ytiles.div(rt);
+    c.y = (rt - c.z * g.ytiles) * g.rows_per_tile;
+    c.rows = min(g.rows_per_tile, p.ny - c.y);
     c.x0 = xt * TX;
     c.w = min(TX, p.nx - c.x0);
     return c;
 }
 
-// The copies of one tile into one stage.  Every warp issues the directions i = warp, warp + NW, ... (i = Q: the
-// flag bytes): the index is warp-uniform, one lane issues.
+// This warp's share of the copies of tile t into one stage: directions i = warp, warp + NW, ... (i = Q: the flag
+// bytes).  The direction index is warp-uniform; lane 0 issues.
 template <int Q, int F, int NT>
 __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__restrict__ A, const Params &p, const BulkGeom &g,
                                                  int t, unsigned stage, unsigned full, int warp, int lane) {
@@ -192,33 +201,41 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     typedef typename Elem<F>::T T;
     constexpr int ES = SH::ES, TX = SH::TX, NW = NT / 32;
     constexpr int n_shift = (Q == 9 ? 6 : Q == 19 ? 10 : 18);               // directions with c_x != 0
+    if (lane != 0) return;
     const bool single = g.tiles_per_row == 1;
     const TileCoord c = tile_coord<TX>(t, g, p);
-    if (lane != 0) return;
-    if (warp == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * c.w * ES + c.w + (single ? 0 : n_shift * SH::PAD)));
+    const int cells = c.rows * c.w;                                         // rows > 1 only if w == nx
+    if (warp == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * cells * ES + cells + (single ? 0 : n_shift * SH::PAD)));
     const long long own = (long long)p.nx * (c.y + (long long)p.ny * c.z);
-    // rows on a y or z face of the box pull some directions from the opposite face (R2): rare, general path
-    const bool face = c.y == 0 || c.y == p.ny - 1 || c.z == 0 || c.z == p.nz - 1;
+    // tiles on a y or z face of the box pull some directions from the opposite face (R2): rare, row by row
+    const bool face = c.y == 0 || c.y + c.rows == p.ny || c.z == 0 || c.z == p.nz - 1;
 #pragma unroll 1
     for (int i = warp; i <= Q; i += NW) {
         if (i == Q) {
-            bulk_g2s(stage + Q * SH::ROWB, p.flags + own + c.x0, (unsigned)c.w, full);
+            bulk_g2s(stage + Q * SH::ROWB, p.flags + own + c.x0, (unsigned)cells, full);
             break;
         }
         const int m = Q == 9 ? d2q9_members[i] : i;
         const int cx = c27_table[m][0];
+        const unsigned dst = stage + i * SH::ROWB + SH::PAD;
         const T *src_row;
         if (!face) {
             src_row = A + own + g.src_off[i];
+            bulk_g2s(dst, src_row + c.x0, (unsigned)(cells * ES), full);
         } else {
-            int ys = c.y - c27_table[m][1], zs = c.z - c27_table[m][2];
-            ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
+            const int cy = c27_table[m][1], cz = c27_table[m][2];
+            int zs = c.z - cz;
             zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
-            src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+            src_row = nullptr;
+#pragma unroll 1
+            for (int r = 0; r < c.rows; ++r) {
+                int ys = c.y + r - cy;
+                ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
+                src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+                bulk_g2s(dst + r * c.w * ES, src_row + c.x0, (unsigned)(c.w * ES), full);
+            }
         }
-        const unsigned dst = stage + i * SH::ROWB + SH::PAD;
-        bulk_g2s(dst, src_row + c.x0, (unsigned)(c.w * ES), full);
-        if (!single && cx != 0) {
+        if (!single && cx != 0) {                                           // multi-tile rows: rows == 1
             if (cx > 0) {                                                   // element x0 - 1: the chunk before x0
                 const int xs = (c.x0 == 0 ? p.nx : c.x0) - SH::HALO_ELEMS;
                 bulk_g2s(dst - SH::PAD, src_row + xs, SH::PAD, full);
@@ -230,8 +247,8 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     }
 }
 
-template <int Q, int F, int NT, int MINB, bool FORCE>
-__global__ void __launch_bounds__(NT, MINB)
+template <int Q, int F, int NT, bool FORCE>
+__global__ void __launch_bounds__(NT, 2)
 stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p,
                            const BulkGeom g) {
     typedef BulkShape<Q, F, NT> SH;
@@ -239,22 +256,24 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
     typedef typename E::T T;
     constexpr int ES = SH::ES, TX = SH::TX, S = SH::S, NW = NT / 32;
     constexpr int SC = PairCodec<F>::SC;
-    static_assert(SH::STAGEB % 16 == 0 && SH::OUTB % 16 == 0 && SH::ROWB % 16 == 0, "bulk copies need 16-byte alignment");
 
     extern __shared__ __align__(128) char smem[];
     const unsigned smem_base = smem_addr(smem);
-    const unsigned bar_full = smem_base + SH::BAR_OFF;
+    const unsigned bar_full = smem_base + SH::BAR_OFF, bar_empty = bar_full + S * 8;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);                  // warp-uniform by construction
 
     if (tid == 0) {
-        for (int s = 0; s < S; ++s) mbar_init(bar_full + s * 8, 1);          // warp 0's arrive.expect_tx
+        for (int s = 0; s < S; ++s) {
+            mbar_init(bar_full + s * 8, 1);                                  // warp 0's arrive.expect_tx
+            mbar_init(bar_empty + s * 8, NW);                                // one arrival per warp
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_async_smem();
     }
     __syncthreads();
 
-    const bool single = g.tiles_per_row == 1;            // the tile is the whole row: x wraps inside the segment
+    const bool single = g.tiles_per_row == 1;            // a tile spans its rows: x wraps inside the segment
     const int stride = gridDim.x;
 
 #pragma unroll 1
@@ -269,70 +288,70 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
         const int s = k % S;
         const unsigned ph = (unsigned)(k / S) & 1u;
         const TileCoord c = tile_coord<TX>(t, g, p);
-        const int y = c.y, z = c.z, x0 = c.x0, w = c.w;
+        const int w = c.w;
         const bool active = xl < w;
         const char *stage = smem + s * SH::STAGEB;
-        char *out = smem + S * SH::STAGEB + (k & 1) * SH::OUTB;
+        const int el = xl - 1 + ((single && xl == 0) ? w : 0);                  // element "xl - 1" of a row
+        const int er = xl + 2 - ((single && xl + 2 == w) ? w : 0);              // element "xl + 2" of a row
 
         mbar_wait(bar_full + s * 8, ph);
-        unsigned fl = 0;
-        if (active) fl = *reinterpret_cast<const unsigned short *>(stage + Q * SH::ROWB + xl);
-        float f[2][Q];
-        const bool fast = active && fl == 0;
-        if (fast) {
-            const int el = xl - 1 + ((single && xl == 0) ? w : 0);              // element "xl - 1"
-            const int er = xl + 2 - ((single && xl + 2 == w) ? w : 0);          // element "xl + 2"
-            const char *base = stage + SH::PAD;
-            PullStaged<Q, F, NT, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f);
-            collide_bgk<Q, FORCE, SC>(f[0], p);
-            collide_bgk<Q, FORCE, SC>(f[1], p);
-#pragma unroll
-            for (int i = 0; i < Q; ++i) {
-                char *o = out + i * SH::OUTROWB + xl * ES;
-                if constexpr (ES == 4) *reinterpret_cast<float2 *>(o) = make_float2(f[0][i], f[1][i]);
-                else *reinterpret_cast<unsigned *>(o) = PairCodec<F>::enc2(f[0][i], f[1][i]);
-            }
-        } else if (active) {
-            // a wall cell or a wall among the pull sources: cell by cell from global memory (lbm_kernels.cuh)
-            const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
-            const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
-            const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
-            long long rows[3][3];
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-#pragma unroll
-                for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
 #pragma unroll 1
-            for (int j = 0; j < 2; ++j) {
-                const int x = x0 + xl + j;
-                T *o = reinterpret_cast<T *>(out) + xl + j;
-                if ((fl >> (8 * j)) & FLAG_WALL) {                              // not updated
+        for (int r = 0; r < c.rows; ++r) {
+            const int y = c.y + r, z = c.z;
+            const long long own = (long long)p.nx * (y + (long long)p.ny * z) + c.x0 + xl;   // the thread's first cell
+            unsigned fl = 0;
+            if (active) fl = *reinterpret_cast<const unsigned short *>(stage + Q * SH::ROWB + r * w + xl);
+            const bool fast = active && fl == 0;
+            float f[2][Q];
+            if (fast) {
+                const char *base = stage + SH::PAD + r * w * ES;
+                PullStaged<Q, F, NT, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f);
+            }
+            if (r + 1 == c.rows) {                                              // the warp has its values in registers:
+                __syncwarp();                                                   // the stage may be refilled
+                if (lane == 0) mbar_arrive(bar_empty + s * 8);
+            }
+            if (fast) {
+                collide_bgk<Q, FORCE, SC>(f[0], p);
+                collide_bgk<Q, FORCE, SC>(f[1], p);
+                T *o = B + own;
 #pragma unroll
-                    for (int i = 0; i < Q; ++i) o[i * TX] = __ldg(A + (long long)i * p.N + rows[1][1] + x);
-                } else {
-                    const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
-                    float gq[Q];
-                    PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, gq);
-                    collide_bgk<Q, FORCE, 0>(gq, p);
+                for (int i = 0; i < Q; ++i) {
+                    if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
+                    else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PairCodec<F>::enc2(f[0][i], f[1][i]);
+                }
+            } else {
+                if (active) {
+                    // a wall cell or a wall among the pull sources: cell by cell from global memory (lbm_kernels.cuh)
+                    const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
+                    const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
+                    const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
+                    long long rows[3][3];
 #pragma unroll
-                    for (int i = 0; i < Q; ++i) E::st1(o + i * TX, gq[i]);
+                    for (int a = 0; a < 3; ++a)
+#pragma unroll
+                        for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
+#pragma unroll 1
+                    for (int j = 0; j < 2; ++j) {
+                        if ((fl >> (8 * j)) & FLAG_WALL) continue;              // wall cells are not updated
+                        const int x = c.x0 + xl + j;
+                        const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
+                        float gq[Q];
+                        PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, gq);
+                        collide_bgk<Q, FORCE, 0>(gq, p);
+#pragma unroll
+                        for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + own + j, gq[i]);
+                    }
                 }
             }
         }
-        fence_async_smem();                                                     // generic-proxy writes -> bulk store
-        if (lane == 0) bulk_wait_read0();                                       // this warp's stores of tile k-1 have left smem
-        __syncthreads();            // everyone has read stage s and written `out`; the other out buffer is free
-        if (lane == 0) {
-            const long long own = (long long)p.nx * (y + (long long)p.ny * z) + x0;
-#pragma unroll 1
-            for (int i = warp; i < Q; i += NW)
-                bulk_s2g(B + (long long)i * p.N + own, smem_addr(out) + i * SH::OUTROWB, (unsigned)(w * ES));
-            bulk_commit();
+        // refill the stage just consumed with tile k+S, once every warp has taken its values out of it
+        const long long tn = (long long)t + (long long)S * stride;
+        if (tn < g.n_tiles) {
+            mbar_wait(bar_empty + s * 8, ph);
+            issue_tile_loads<Q, F, NT>(A, p, g, (int)tn, smem_base + s * SH::STAGEB, bar_full + s * 8, warp, lane);
         }
-        const long long tn = (long long)t + (long long)S * stride;              // refill the stage just consumed
-        if (tn < g.n_tiles) issue_tile_loads<Q, F, NT>(A, p, g, (int)tn, smem_base + s * SH::STAGEB, bar_full + s * 8, warp, lane);
     }
-    if (lane == 0) bulk_wait0();
 }
 
 }  // namespace lbmk

@@ -35,15 +35,27 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
 
 
 // ---- the shared-memory-staged variant (lbm_bulk.cuh) ------------------------------------------------
-// consumer threads per CTA and CTAs per SM, by velocity set: shared memory per CTA is
-// S*(Q*(2*NT*ES+32)+2*NT) + 2*Q*2*NT*ES bytes
-constexpr int BULK_NT = Q == 27 ? 128 : (Elem<F>::SIZE == 4 ? 128 : 256);
-constexpr int BULK_MINB = Q == 9 ? 3 : Q == 19 ? 2 : 3;
+constexpr int BULK_NT = 256;
+
+BulkGeom bulk_geom(const Params &p, long long *tiles) {
+    typedef BulkShape<Q, F, BULK_NT> SH;
+    BulkGeom g;
+    g.tiles_per_row = (p.nx + SH::TX - 1) / SH::TX;
+    g.rows_per_tile = g.tiles_per_row == 1 ? SH::RMAX : 1;
+    g.ytiles = (p.ny + g.rows_per_tile - 1) / g.rows_per_tile;
+    *tiles = (long long)g.tiles_per_row * g.ytiles * p.nz;
+    g.n_tiles = (int)(*tiles < 0x7FFFFFFFLL ? *tiles : 0x7FFFFFFFLL);
+    g.by_tpr = FastDiv::make(g.tiles_per_row);
+    g.by_ytiles = FastDiv::make(g.ytiles);
+    for (int i = 0; i < 27; ++i)
+        g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
+    return g;
+}
 
 template <bool FORCE>
 cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st) {
     typedef BulkShape<Q, F, BULK_NT> SH;
-    auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, BULK_MINB, FORCE>;
+    auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, FORCE>;
     static int ctas = 0;                      // resident CTAs on the device, resolved once per instantiation
     if (ctas == 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SH::SMEM);
@@ -55,15 +67,9 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
         ctas = sms * per_sm;
     }
-    BulkGeom g;
-    g.tiles_per_row = (p.nx + SH::TX - 1) / SH::TX;
-    const long long tiles = (long long)g.tiles_per_row * p.ny * p.nz;
+    long long tiles = 0;
+    const BulkGeom g = bulk_geom(p, &tiles);
     if (p.nx % 16 != 0 || tiles > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
-    g.n_tiles = (int)tiles;
-    g.by_tpr = FastDiv::make(g.tiles_per_row);
-    g.by_ny = FastDiv::make(p.ny);
-    for (int i = 0; i < 27; ++i)
-        g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
     const int grid = (int)(tiles < ctas ? tiles : ctas);
     kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g);
     count_launch();

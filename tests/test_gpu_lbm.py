@@ -153,33 +153,39 @@ BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16
                (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1))]
 
 
+STAGED = [(lbm.VARIANT_BULK, "bulk")]
+
+
 @pytest.mark.parametrize("q,shape", BULK_SHAPES)
 @pytest.mark.parametrize("name", ALL_FORMATS)
-def test_bulk_variant_periodic(q, shape, name):
+@pytest.mark.parametrize("variant,tag", STAGED)
+def test_bulk_variant_periodic(q, shape, name, variant, tag):
     w = wl.perturbed_equilibrium(*shape, seed=21, velset=q)
-    osim, gsim = run_pair(w, name, 12, variant=lbm.VARIANT_BULK)
-    assert "bulk" in gsim.kernel_name
+    osim, gsim = run_pair(w, name, 12, variant=variant)
+    assert tag in gsim.kernel_name
     assert_parity(osim, gsim, name)
 
 
 @pytest.mark.parametrize("q,shape", [(19, (48, 7, 5)), (19, (544, 3, 3)), (27, (32, 6, 5)), (9, (64, 11, 1))])
 @pytest.mark.parametrize("name", ALL_FORMATS)
-def test_bulk_variant_walls_moving_walls_force(q, shape, name):
+@pytest.mark.parametrize("variant,tag", STAGED)
+def test_bulk_variant_walls_moving_walls_force(q, shape, name, variant, tag):
     w = wl.perturbed_equilibrium(*shape, seed=23, velset=q, tau=0.7)
     w = wl.random_walls(w, 0.12, seed=29, moving_fraction=0.5)
     w.force = (1e-5, -2e-5, 0.0 if q == 9 else 3e-5)
-    osim, gsim = run_pair(w, name, 25, variant=lbm.VARIANT_BULK)
-    assert "bulk" in gsim.kernel_name
+    osim, gsim = run_pair(w, name, 25, variant=variant)
+    assert tag in gsim.kernel_name
     assert_parity(osim, gsim, name)
 
 
 @pytest.mark.parametrize("name", ["FP16S", "FP16C", "P16_0S"])
-def test_bulk_variant_taylor_green_and_cavity(name):
+@pytest.mark.parametrize("variant,tag", STAGED)
+def test_bulk_variant_taylor_green_and_cavity(name, variant, tag):
     w = wl.taylor_green_3d(32)
-    osim, gsim = run_pair(w, name, 200, variant=lbm.VARIANT_BULK)
+    osim, gsim = run_pair(w, name, 200, variant=variant)
     assert_parity(osim, gsim, name)
     w = wl.lid_driven_cavity(32, tau=0.5384)
-    osim, gsim = run_pair(w, name, 300, variant=lbm.VARIANT_BULK)
+    osim, gsim = run_pair(w, name, 300, variant=variant)
     assert_parity(osim, gsim, name)
 
 
