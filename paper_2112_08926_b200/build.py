@@ -24,7 +24,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblbm_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ARCH + ["-O3", "-std=c++17", "-lineinfo", "--fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
+FLAGS = ARCH + (["-DLBM_SELFTEST_DEBUG"] if os.environ.get("LBM_SELFTEST_DEBUG") else []) + ["-O3", "-std=c++17", "-lineinfo", "--fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
                 "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-Xptxas", "-v"]
 VELSETS = (9, 19, 27)
 FORMATS = (0, 1, 2, 3, 4, 5, 6)

@@ -1,6 +1,7 @@
 // lbm_aux.cu -- small kernels beside the hot path: the FLAG_NEAR pass of lbm_set_flags and the
 // stand-alone codec kernels behind lbm_codec_encode / lbm_codec_decode (bit-level parity tests).
 #include <atomic>
+#include <cstdio>
 
 #include "lbm_internal.h"
 #include "lbm_kernels.cuh"
@@ -82,32 +83,112 @@ cudaError_t launch_codec(int fmt, bool encode, const void *in, void *out, long l
     return cudaErrorInvalidValue;
 }
 
+// ---- encoder tables of the table-driven pair codecs (lbm_codecs.cuh, "posits on pairs") -----------------
+// One entry per (sign, FP32 exponent) of the encoder's input X = 2^SC x, derived from Codec<F>::enc itself:
+//   c0, c1 = codes of the first and last value of the binade; d = c1 - c0
+//   d = 0        constant code                                      -> mult = 1 (hi32 = 0)
+//   d = 1        one threshold, found by bisection (enc is monotone) -> (M + 2^23 - thr) >> 23
+//   d = 2^nf     nf fraction bits, round half up                     -> (M + 2^(22-nf)) >> (23-nf)
+//   d = 2^nf - 1 and c1 saturated (0x7FFF): same, with M + add bounded so the top half step stays at 0x7FFF
+// anything else would make the entry unusable: mult = 0 marks it and lbm_codec_pair_selftest reports it.
+__device__ EncEntry g_enc_tables[7][512];
+
+template <int F>
+__global__ void __launch_bounds__(512) enc_table_kernel(EncEntry *tab) {
+    const unsigned idx = threadIdx.x;
+    const float dn = pow2f(-PairCodec<F>::SC);
+    auto probe = [&](unsigned M) { return Codec<F>::enc(__fmul_rn(__uint_as_float((idx << 23) | M), dn)); };
+    // exponent 255: M = 0 is infinity (saturates), M != 0 a NaN, whose code is not pinned: the binade gets infinity's code
+    const unsigned c0 = probe(0), c1 = (idx & 255u) == 255u ? c0 : probe(0x7FFFFFu), d = c1 - c0;
+    EncEntry e;
+    e.base = c0;
+    e.tmax = 0xFFFFFFFFu;
+    unsigned add = 0;
+    if (d == 0) {
+        e.mult = 1u;
+    } else if (d == 1) {
+        unsigned lo = 0, hi = 0x7FFFFFu;                    // probe(lo) = c0, probe(hi) = c1
+        while (hi - lo > 1) {
+            const unsigned mid = (lo + hi) >> 1;
+            if (probe(mid) == c0) lo = mid; else hi = mid;
+        }
+        add = (1u << 23) - hi;
+        e.mult = 1u << 9;
+    } else if ((d & (d - 1)) == 0 || (((d + 1) & d) == 0 && (c1 & 0x7FFFu) == 0x7FFFu)) {
+        const bool sat = (d & (d - 1)) != 0;
+        const int nf = 31 - __clz((int)(sat ? d + 1 : d)), sh = 23 - nf;
+        add = 1u << (sh - 1);
+        e.mult = 1u << (32 - sh);
+        if (sat) e.tmax = (d << sh) | ((1u << sh) - 1u);
+    } else {
+        e.mult = 0u;
+#ifdef LBM_SELFTEST_DEBUG
+        printf("enc_table F=%d idx=%u c0=%04x c1=%04x\n", F, idx, c0, c1);
+#endif
+    }
+    e.add = add - (idx << 23);
+    tab[idx] = e;
+}
+
+cudaError_t enc_table(int fmt, const EncEntry **out, cudaStream_t st) {
+    static bool built[64][7];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    EncEntry *base = nullptr;
+    if ((e = cudaGetSymbolAddress((void **)&base, g_enc_tables)) != cudaSuccess) return e;
+    EncEntry *tab = base + fmt * 512;
+    *out = tab;
+    if (dev < 0 || dev >= 64 || fmt < 0 || fmt > 6) return cudaErrorInvalidValue;
+    if (built[dev][fmt]) return cudaSuccess;
+    switch (fmt) {
+        case F_P16_0S: enc_table_kernel<F_P16_0S><<<1, 512, 0, st>>>(tab); break;
+        case F_P16_1S: enc_table_kernel<F_P16_1S><<<1, 512, 0, st>>>(tab); break;
+        case F_P16_2C: enc_table_kernel<F_P16_2C><<<1, 512, 0, st>>>(tab); break;
+        default: return cudaSuccess;                        // formats without a table
+    }
+    count_launch();
+    built[dev][fmt] = true;
+    return cudaGetLastError();
+}
+
 // ---- pair codecs vs scalar codecs, exhaustively, on the device ----------------------------------------
 // PairCodec<F> (the staged kernel's converters) must return bit for bit what Codec<F> returns (times 2^SC):
 // all 65 536 codes through dec1 / dec2 (both halves) and ALL 2^32 FP32 bit patterns through enc2 (both halves).
 // Codec<F> itself is compared with the oracle by the tests; this closes the chain for PairCodec<F>.
 template <int F>
-__global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *mismatches) {
+__global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *mismatches, const EncEntry *tab) {
     typedef PairCodec<F> PC;
     const float up = pow2f(PC::SC);
     unsigned long long bad = 0;
+    if (PC::TABLE)
+        for (int i = 0; i < 512; ++i) bad += tab[i].mult == 0;                 // an entry the table kernel could not express
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
     for (unsigned long long v = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; v < (1ull << 32); v += stride) {
         const unsigned b = (unsigned)v;
         const float x = __uint_as_float(b);
         const float other = __uint_as_float(b * 2654435761u + 12345u);          // an unrelated partner value
         const unsigned ref = Codec<F>::enc(x), ref_o = Codec<F>::enc(other);
-        const unsigned w1 = PC::enc2(__fmul_rn(x, up), __fmul_rn(other, up));
-        const unsigned w2 = PC::enc2(__fmul_rn(other, up), __fmul_rn(x, up));
+        const unsigned w1 = PC::enc2(__fmul_rn(x, up), __fmul_rn(other, up), tab);
+        const unsigned w2 = PC::enc2(__fmul_rn(other, up), __fmul_rn(x, up), tab);
         const bool nan = x != x || other != other;                              // NaN payloads of binary16 are not pinned
         if (!nan) bad += (w1 != (ref | (ref_o << 16))) + (w2 != (ref_o | (ref << 16)));
+#ifdef LBM_SELFTEST_DEBUG
+        if (!nan && (w1 & 0xFFFFu) != ref && (b % 977u) == 0) printf("enc x=%08x ref=%04x got=%04x\n", b, ref, w1 & 0xFFFFu);
+#endif
         if (v < 65536) {
-            const unsigned c = (unsigned)v, c2 = (c * 40503u + 7u) & 0xFFFFu;
+            unsigned c = (unsigned)v, c2 = (c * 40503u + 7u) & 0xFFFFu;
+            if (PC::CHECK) { c2 &= ~PC::CHECK; if (c & PC::CHECK) continue; }  // outside the fast decoders' domain: the kernel falls back
             const float r = __fmul_rn(Codec<F>::dec(c), up), r2 = __fmul_rn(Codec<F>::dec(c2), up);
             float a, d;
             PC::dec2(c | (c2 << 16), a, d);
             const float e = PC::dec1((int)(short)c);
             const bool cn = r != r || r2 != r2;
+#ifdef LBM_SELFTEST_DEBUG
+            if (!cn && __float_as_uint(a) != __float_as_uint(r)) printf("dec2lo c=%04x ref=%08x got=%08x\n", c, __float_as_uint(r), __float_as_uint(a));
+            if (!cn && __float_as_uint(e) != __float_as_uint(r)) printf("dec1 c=%04x ref=%08x got=%08x\n", c, __float_as_uint(r), __float_as_uint(e));
+            if (!cn && __float_as_uint(d) != __float_as_uint(r2)) printf("dec2hi c=%04x ref=%08x got=%08x\n", c2, __float_as_uint(r2), __float_as_uint(d));
+#endif
             if (cn) bad += !(a != a || !(r != r)) + !(d != d || !(r2 != r2)) + !(e != e || !(r != r));
             else bad += (__float_as_uint(a) != __float_as_uint(r)) + (__float_as_uint(d) != __float_as_uint(r2)) +
                         (__float_as_uint(e) != __float_as_uint(r));
@@ -118,13 +199,16 @@ __global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *
 
 cudaError_t launch_pair_selftest(int fmt, unsigned long long *mismatches_dev, cudaStream_t st) {
     const int blocks = 148 * 16;
+    const EncEntry *tab = nullptr;
+    cudaError_t e = enc_table(fmt, &tab, st);
+    if (e != cudaSuccess) return e;
     switch (fmt) {
-        case F_FP16S: pair_selftest_kernel<F_FP16S><<<blocks, 256, 0, st>>>(mismatches_dev); break;
-        case F_FP16C: pair_selftest_kernel<F_FP16C><<<blocks, 256, 0, st>>>(mismatches_dev); break;
-        case F_P16_0S: pair_selftest_kernel<F_P16_0S><<<blocks, 256, 0, st>>>(mismatches_dev); break;
-        case F_P16_1S: pair_selftest_kernel<F_P16_1S><<<blocks, 256, 0, st>>>(mismatches_dev); break;
-        case F_P16_2C: pair_selftest_kernel<F_P16_2C><<<blocks, 256, 0, st>>>(mismatches_dev); break;
-        case F_FP16: pair_selftest_kernel<F_FP16><<<blocks, 256, 0, st>>>(mismatches_dev); break;
+        case F_FP16S: pair_selftest_kernel<F_FP16S><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
+        case F_FP16C: pair_selftest_kernel<F_FP16C><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
+        case F_P16_0S: pair_selftest_kernel<F_P16_0S><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
+        case F_P16_1S: pair_selftest_kernel<F_P16_1S><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
+        case F_P16_2C: pair_selftest_kernel<F_P16_2C><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
+        case F_FP16: pair_selftest_kernel<F_FP16><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
         default: return cudaErrorInvalidValue;
     }
     count_launch();

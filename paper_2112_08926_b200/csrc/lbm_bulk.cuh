@@ -118,15 +118,17 @@ struct BulkShape {
     static constexpr int TX = 2 * NT;                   // cells per tile row
     static constexpr int PAD = 16;                      // halo pad in front of and behind every segment
     static constexpr int MAXB = (227 * 1024 - 2048) / 2;                    // two CTAs per SM
+    static constexpr int TABB = PairCodec<F>::TABLE ? 512 * 16 : 0;        // the format's encoder table
     static constexpr int row_stage(int r) { return Q * (r * TX * ES + 2 * PAD) + r * TX; }
-    static constexpr int RMAX = 2 * row_stage(2) <= MAXB ? 2 : 1;           // rows per tile (single-tile rows only)
+    static constexpr int RMAX = 2 * row_stage(2) + TABB <= MAXB ? 2 : 1;    // rows per tile (single-tile rows only)
     static constexpr int ROWB = RMAX * TX * ES + 2 * PAD;                   // one direction of one stage
     static constexpr int STAGEB = row_stage(RMAX);                          // + the tile's flag bytes
-    static constexpr int S = 3 * STAGEB <= MAXB ? 3 : 2;                    // input stages
-    static constexpr int BAR_OFF = S * STAGEB;
+    static constexpr int S = 3 * STAGEB + TABB <= MAXB ? 3 : 2;             // input stages
+    static constexpr int TAB_OFF = S * STAGEB;
+    static constexpr int BAR_OFF = TAB_OFF + TABB;
     static constexpr int SMEM = BAR_OFF + 2 * S * 8;                        // full[S], empty[S]
     static constexpr int HALO_ELEMS = PAD / ES;                             // elements in one 16-byte halo copy
-    static_assert(2 * STAGEB <= MAXB, "two stages of two CTAs must fit one SM");
+    static_assert(2 * STAGEB + TABB <= MAXB, "two stages of two CTAs must fit one SM");
     static_assert(STAGEB % 16 == 0 && ROWB % 16 == 0, "bulk copies need 16-byte alignment");
 };
 
@@ -138,11 +140,12 @@ __device__ __forceinline__ float lds_f32(const char *p) { return *reinterpret_ca
 // the two values of direction I for the thread's cells xl, xl+1, from the staged segment.
 //   own  = address of element xl of direction 0's segment; left = element "xl - 1", right = element "xl + 2"
 //   (already wrapped / pointing into the pads); direction I adds the immediate I * ROWB.
-template <int Q, int F, int NT, int I>
+template <int Q, int F, int NT, class PC, int I>
 struct PullStaged {
     typedef BulkShape<Q, F, NT> SH;
-    typedef PairCodec<F> PC;
-    static __device__ __forceinline__ void run(const char *own, const char *left, const char *right, float (&f)[2][Q]) {
+    // acc collects the raw words (pairs in both halves, single codes in the low half) for PairCodec<F>::CHECK
+    static __device__ __forceinline__ void run(const char *own, const char *left, const char *right, float (&f)[2][Q],
+                                               unsigned &acc) {
         typedef Lat<Q> L;
         constexpr int cx = L::c(I, 0);
         constexpr int o = I * SH::ROWB;
@@ -160,21 +163,23 @@ struct PullStaged {
             }
         } else {
             if (cx == 0) {
-                PC::dec2(lds_u32(own + o), f[0][I], f[1][I]);
-            } else if (cx > 0) {
-                f[0][I] = PC::dec1(lds_s16(left + o));
-                f[1][I] = PC::dec1(lds_s16(own + o));
+                const unsigned w = lds_u32(own + o);
+                if (PC::CHECK) acc |= w;
+                PC::dec2(w, f[0][I], f[1][I]);
             } else {
-                f[0][I] = PC::dec1(lds_s16(own + o + 2));
-                f[1][I] = PC::dec1(lds_s16(right + o));
+                const int c0 = lds_s16(cx > 0 ? left + o : own + o + 2);
+                const int c1 = lds_s16(cx > 0 ? own + o : right + o);
+                if (PC::CHECK) acc |= (unsigned)(c0 | c1) & 0xFFFFu;
+                f[0][I] = PC::dec1(c0);
+                f[1][I] = PC::dec1(c1);
             }
         }
-        PullStaged<Q, F, NT, I + 1>::run(own, left, right, f);
+        PullStaged<Q, F, NT, PC, I + 1>::run(own, left, right, f, acc);
     }
 };
-template <int Q, int F, int NT>
-struct PullStaged<Q, F, NT, Q> {
-    static __device__ __forceinline__ void run(const char *, const char *, const char *, float (&)[2][Q]) {}
+template <int Q, int F, int NT, class PC>
+struct PullStaged<Q, F, NT, PC, Q> {
+    static __device__ __forceinline__ void run(const char *, const char *, const char *, float (&)[2][Q], unsigned &) {}
 };
 
 struct TileCoord {
@@ -250,12 +255,13 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
 template <int Q, int F, int NT, bool FORCE>
 __global__ void __launch_bounds__(NT, 2)
 stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p,
-                           const BulkGeom g) {
+                           const BulkGeom g, const EncEntry *__restrict__ enc_table) {
     typedef BulkShape<Q, F, NT> SH;
     typedef Elem<F> E;
     typedef typename E::T T;
     constexpr int ES = SH::ES, TX = SH::TX, S = SH::S, NW = NT / 32;
-    constexpr int SC = PairCodec<F>::SC;
+    typedef PairCodec<F> PC;
+    constexpr int SC = PC::SC;
 
     extern __shared__ __align__(128) char smem[];
     const unsigned smem_base = smem_addr(smem);
@@ -270,6 +276,11 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_async_smem();
+    }
+    const EncEntry *tab = reinterpret_cast<const EncEntry *>(smem + SH::TAB_OFF);
+    if constexpr (PC::TABLE) {
+        for (int i = tid; i < 512; i += NT)
+            reinterpret_cast<uint4 *>(smem + SH::TAB_OFF)[i] = __ldg(reinterpret_cast<const uint4 *>(enc_table) + i);
     }
     __syncthreads();
 
@@ -303,22 +314,35 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             if (active) fl = *reinterpret_cast<const unsigned short *>(stage + Q * SH::ROWB + r * w + xl);
             const bool fast = active && fl == 0;
             float f[2][Q];
-            if (fast) {
-                const char *base = stage + SH::PAD + r * w * ES;
-                PullStaged<Q, F, NT, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f);
+            unsigned acc = 0;
+            const char *base = stage + SH::PAD + r * w * ES;
+            if (fast) PullStaged<Q, F, NT, PC, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
+            // codes outside the fast decoders' domain (posits: a regime of ones): this pair goes through Codec<F>
+            const bool exact = PC::CHECK != 0 && ((acc | (acc >> 16)) & PC::CHECK) != 0;
+            if (exact) {
+                unsigned dummy = 0;
+                PullStaged<Q, F, NT, PairCodec<-1 - F>, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, dummy);
             }
             if (r + 1 == c.rows) {                                              // the warp has its values in registers:
                 __syncwarp();                                                   // the stage may be refilled
                 if (lane == 0) mbar_arrive(bar_empty + s * 8);
             }
             if (fast) {
-                collide_bgk<Q, FORCE, SC>(f[0], p);
-                collide_bgk<Q, FORCE, SC>(f[1], p);
                 T *o = B + own;
+                if (!exact) {
+                    collide_bgk<Q, FORCE, SC>(f[0], p);
+                    collide_bgk<Q, FORCE, SC>(f[1], p);
 #pragma unroll
-                for (int i = 0; i < Q; ++i) {
-                    if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
-                    else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PairCodec<F>::enc2(f[0][i], f[1][i]);
+                    for (int i = 0; i < Q; ++i) {
+                        if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
+                        else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PC::enc2(f[0][i], f[1][i], tab);
+                    }
+                } else if constexpr (ES == 2) {
+                    collide_bgk<Q, FORCE, 0>(f[0], p);
+                    collide_bgk<Q, FORCE, 0>(f[1], p);
+#pragma unroll
+                    for (int i = 0; i < Q; ++i)
+                        *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = Codec<F>::enc(f[0][i]) | (Codec<F>::enc(f[1][i]) << 16);
                 }
             } else {
                 if (active) {

@@ -157,28 +157,41 @@ struct Codec<F_P16_2C> {
 //             anyway -- decode is one HADD2.F32, encode half an F2FP.PACK_AB per value;
 //   dec1(c)   c = one code SIGN-EXTENDED to 32 bits (ld.shared.s16);
 //   dec2(w)   both codes of a word;  enc2(a, b) packs the codes of a (low) and b (high).
+//   TABLE     enc2 reads the format's 512-entry encoder table (EncEntry, below) from shared memory;
+//   CHECK     codes with (code & CHECK) != 0 are outside the domain of dec1 / dec2: the caller ORs the raw words
+//             together and, if a CHECK bit shows up, redoes the cell with Codec<F> (rare by construction).
 // Every function returns bit for bit what Codec<F>::dec / enc return (times 2^SC).
+struct EncEntry {
+    unsigned add, mult, base, tmax;     // code = base + hi32(min(bits(X) + add, tmax) * mult)
+};
+
 template <int F>
 struct PairCodec {
     static constexpr int SC = 0;
+    static constexpr bool TABLE = false;
+    static constexpr unsigned CHECK = 0;
     static __device__ __forceinline__ float dec1(int c) { return Codec<F>::dec((unsigned)c & 0xFFFFu); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
         a = Codec<F>::dec(w & 0xFFFFu);
         b = Codec<F>::dec(w >> 16);
     }
-    static __device__ __forceinline__ unsigned enc2(float a, float b) { return Codec<F>::enc(a) | (Codec<F>::enc(b) << 16); }
+    static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *) {
+        return Codec<F>::enc(a) | (Codec<F>::enc(b) << 16);
+    }
 };
 
 template <int SCALE>
 struct PairHalf {
     static constexpr int SC = SCALE;
+    static constexpr bool TABLE = false;
+    static constexpr unsigned CHECK = 0;
     static __device__ __forceinline__ float dec1(int c) { return __half2float(__ushort_as_half((unsigned short)c)); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
         const float2 v = __half22float2(*reinterpret_cast<const __half2 *>(&w));
         a = v.x;
         b = v.y;
     }
-    static __device__ __forceinline__ unsigned enc2(float a, float b) {
+    static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *) {
         const __half2 h = __floats2half2_rn(a, b);          // one F2FP.F16.F32.PACK_AB, round-to-nearest-even
         return *reinterpret_cast<const unsigned *>(&h);
     }
@@ -196,6 +209,8 @@ struct PairCodec<F_FP16S> : PairHalf<15> {};
 template <>
 struct PairCodec<F_FP16C> {
     static constexpr int SC = 0;
+    static constexpr bool TABLE = false;
+    static constexpr unsigned CHECK = 0;
     static __device__ __forceinline__ float bits2f(unsigned t) {
         return __fmul_rn(__uint_as_float(t & 0x87FFF000u), __uint_as_float(0x77800000u));   // * 2^112, exact
     }
@@ -208,11 +223,102 @@ struct PairCodec<F_FP16C> {
         const float y = __fmul_rz(fminf(fabsf(x), __uint_as_float(0x3FFFF000u) /* 2 - 2^-11 */), __uint_as_float(0x07800000u));
         return (__float_as_uint(y) + 0x800u) << 4;
     }
-    static __device__ __forceinline__ unsigned enc2(float a, float b) {
+    static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *) {
         const unsigned mags = __byte_perm(mag4(a), mag4(b), 0x7632);
         const unsigned signs = __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x7632);
         return (mags & 0x7FFF7FFFu) | (signs & 0x80008000u);
     }
 };
+
+// ---- posits on pairs ------------------------------------------------------------------------------------
+// Encode, all three posits: the code of X = +-2^E (1 + M 2^-23) is, inside one binade, base(E) plus the rounded
+// leading fraction bits of M -- and where the regime leaves no fraction bits, base(E) plus one step at one
+// threshold.  Both are  base + ((M + add) >> sh)  with per-binade constants (carries run from the fraction into
+// exponent and regime because posit codes are monotone; the paper's converters use the same
+// fact).  The 512 (sign, exponent) entries are derived ON THE DEVICE from Codec<F>::enc
+// (enc_table_kernel, lbm_aux.cu) and then checked against it on all 2^32 inputs (lbm_codec_pair_selftest).
+// One table read, one add and one multiply-high replace the regime arithmetic; sign, scaling (2^7 for P16_0S /
+// P16_1S), saturation and the nearest-value corners of DESIGN.md R14 are all inside the table.
+// CLAMP: the top binade of an unscaled format ends in the saturating code (P16_2C: [1, 2) -> 0x7000..0x7FFF): the
+// entry's fourth word bounds (M + add) so that values within half a step of 2 stay at 0x7FFF.
+template <bool CLAMP>
+__device__ __forceinline__ unsigned enc_by_table(float X, const EncEntry *tab) {
+    const unsigned xb = __float_as_uint(X);
+    const uint4 e = *reinterpret_cast<const uint4 *>(tab + (xb >> 23));
+    unsigned t = xb + e.x;
+    if (CLAMP) t = min(t, e.w);
+    return __umulhi(t, e.y) + e.z;
+}
+
+// Decode for a regime of ZEROS (value below 1 before scaling; P16_2C has no other kind).  The 15 magnitude bits
+// "0..01 e F" read as an integer n are 2^(14-k) (1 + [e F]): normalising n (one multiply of the FP32 denormal
+// n 2^-141 by 2^127) yields exponent field 127-k and the bits [e F] left-aligned in the mantissa, which is the
+// posit's value up to a fixed affine map of the FP32 word:
+//   es = 0   value = n 2^-14 exactly -- posits with es = 0 are linear below 1;
+//   es = 1   word = 2 b - 0x43000000        (exponent field 120 - 2k + e, scale 2^-7 included);
+//   es = 2   word = 4 b + 0x40000000        (exponent field 124 - 4r + e; mod 2^32);
+// max(b, .) maps the zero code to zero.  A regime of ONES (bit 14 set, |f| >= 2^-7) is not handled here: CHECK.
+template <>
+struct PairCodec<F_P16_0S> {
+    static constexpr int SC = -1;           // decoded = n 2^-22 = f / 2: one multiply, the factor 2 rides on SC
+    static constexpr bool TABLE = true;
+    static constexpr unsigned CHECK = 0x4000u;
+    static __device__ __forceinline__ float sm2f(unsigned t) {      // t = sign-extended code
+        return __fmul_rn(__uint_as_float(t & 0x80007FFFu), __uint_as_float(0x7F000000u));   // * 2^127, exact
+    }
+    static __device__ __forceinline__ float dec1(int c) { return sm2f((unsigned)c); }
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        a = sm2f(__byte_perm(w, 0, 0x9910));                        // sign-extend the low half-word
+        b = sm2f((unsigned)((int)w >> 16));
+    }
+    static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *tab) {
+        return __byte_perm(enc_by_table<false>(a, tab), enc_by_table<false>(b, tab), 0x5410);
+    }
+};
+
+template <int MUL, unsigned OFF, unsigned FLOOR, unsigned CHK>
+struct PairPositLow {
+    static constexpr int SC = 0;
+    static constexpr bool TABLE = true;
+    static constexpr unsigned CHECK = CHK;
+    // t = the code shifted so that the magnitude sits in bits 22..8 and the sign in bit 31
+    static __device__ __forceinline__ float word(unsigned t) {
+        const unsigned b = __float_as_uint(__fmul_rn(__uint_as_float(t & 0x007FFF00u), __uint_as_float(0x7F000000u)));
+        const unsigned v = max(b, FLOOR) * (unsigned)MUL + OFF;
+        return __uint_as_float(v | (t & 0x80000000u));
+    }
+    static __device__ __forceinline__ float dec1(int c) { return word((unsigned)c << 8); }     // c sign-extended
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        a = word(__byte_perm(w, 0, 0x9910) << 8);
+        b = word((unsigned)((int)w >> 8));
+    }
+    static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *tab) {
+        return __byte_perm(enc_by_table<CHK == 0>(a, tab), enc_by_table<CHK == 0>(b, tab), 0x5410);
+    }
+};
+template <>
+struct PairCodec<F_P16_1S> : PairPositLow<2, 0xBD000000u /* -0x43000000 */, 0x21800000u, 0x4000u> {};
+template <>
+struct PairCodec<F_P16_2C> : PairPositLow<4, 0x40000000u, 0x30000000u, 0u> {};
+
+// PairCodec<-1 - F>: the exact fall-back decoders (Codec<F> on every code), used when a CHECK bit shows up
+template <int F>
+struct ExactPair {
+    static constexpr int SC = 0;
+    static constexpr bool TABLE = false;
+    static constexpr unsigned CHECK = 0;
+    static __device__ __forceinline__ float dec1(int c) { return Codec<F>::dec((unsigned)c & 0xFFFFu); }
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        a = Codec<F>::dec(w & 0xFFFFu);
+        b = Codec<F>::dec(w >> 16);
+    }
+};
+template <> struct PairCodec<-1 - F_FP16S> : ExactPair<F_FP16S> {};
+template <> struct PairCodec<-1 - F_FP16C> : ExactPair<F_FP16C> {};
+template <> struct PairCodec<-1 - F_P16_0S> : ExactPair<F_P16_0S> {};
+template <> struct PairCodec<-1 - F_P16_1S> : ExactPair<F_P16_1S> {};
+template <> struct PairCodec<-1 - F_P16_2C> : ExactPair<F_P16_2C> {};
+template <> struct PairCodec<-1 - F_FP16> : ExactPair<F_FP16> {};
+template <> struct PairCodec<-1 - F_FP32> : ExactPair<F_FP16> {};       // never used (FP32 has no codes); keeps templates well-formed
 
 }  // namespace lbmk

@@ -71,7 +71,12 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
     const BulkGeom g = bulk_geom(p, &tiles);
     if (p.nx % 16 != 0 || tiles > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
     const int grid = (int)(tiles < ctas ? tiles : ctas);
-    kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g);
+    const EncEntry *tab = nullptr;
+    if (PairCodec<F>::TABLE) {
+        cudaError_t e = enc_table(F, &tab, st);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g, tab);
     count_launch();
     return cudaGetLastError();
 }
