@@ -198,3 +198,63 @@ def test_automatic_variant_choice():
     assert "bulk" not in lbm.from_workload(w, "FP16S").kernel_name
     with pytest.raises(lbm.LbmError):
         lbm.from_workload(w, "FP16S", variant=lbm.VARIANT_BULK)
+
+
+# ---- BASELINE.json's full size, in the launch configuration bench.py times ---------------------------
+# 512^3 D3Q19 periodic, perturbed equilibrium, automatic kernel choice (per-thread kernel for FP32, staged kernel
+# with persistent CTAs and two-row tiles for the 16-bit formats).  The oracle cannot step 134 M cells in
+# seconds, but after n steps a cell depends only on the initial fields within n cells of it: sampled blocks of
+# 14^3 cells (some straddling the periodic faces) are stepped by the oracle as small boxes of their own and
+# their cores, 8^3 cells each at distance >= 3 from the block's faces, must agree with the GPU bit for bit.
+FULL_L, FULL_STEPS, BLK = 512, 3, 14
+
+
+@pytest.fixture(scope="module")
+def full_size_workload():
+    return wl.perturbed_equilibrium(FULL_L, FULL_L, FULL_L, seed=20211208, tau=0.6)
+
+
+def _block(field, origin, L):
+    """field [..., z, y, x] -> the BLK^3 block starting at origin (x, y, z), periodic."""
+    ix = [np.arange(o, o + BLK) % L for o in origin]
+    return field[..., ix[2][:, None, None], ix[1][None, :, None], ix[0][None, None, :]]
+
+
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "FP16C", "P16_0S", "P16_1S", "P16_2C"])
+def test_full_size_sampled_blocks(full_size_workload, name):
+    w, L = full_size_workload, FULL_L
+    g = lbm.from_workload(w, name)
+    assert ("bulk" in g.kernel_name) == (name != "FP32")
+    g.step(FULL_STEPS)
+    grho, gu = g.read_rho_u()
+    g.close()
+    assert np.all(np.isfinite(grho))
+    grho = grho.reshape(L, L, L)
+    gu = gu.reshape(3, L, L, L)
+    rho0 = w.rho.reshape(L, L, L)
+    u0 = w.u.reshape(3, L, L, L)
+    rng = np.random.default_rng(5)
+    origins = [(-7, -7, -7), (L - 7, 100, 200), (300, L - 7, 17), (40, 50, L - 7), (0, 0, 0), (249, 255, 511 - 13)]
+    origins += [tuple(int(v) for v in rng.integers(0, L, 3)) for _ in range(6)]
+    c = slice(3, BLK - 3)
+    for o in origins:
+        sub = wl.Workload("block", BLK, BLK, BLK, 19, w.tau, np.ascontiguousarray(_block(rho0, o, L)).reshape(-1),
+                          np.ascontiguousarray(_block(u0, o, L)).reshape(3, -1), np.zeros(BLK ** 3, np.uint8))
+        osim = oracle.from_workload(sub, FORMATS[name])
+        osim.step(FULL_STEPS)
+        orho, ou = osim.read_rho_u()
+        orho = orho.reshape(BLK, BLK, BLK)[c, c, c]
+        ou = ou.reshape(3, BLK, BLK, BLK)[:, c, c, c]
+        assert np.array_equal(_block(grho, o, L)[c, c, c].view(np.uint32), orho.view(np.uint32)), (name, o)
+        assert np.array_equal(_block(gu, o, L)[:, c, c, c].view(np.uint32), ou.view(np.uint32)), (name, o)
+
+
+def test_full_size_mass_conservation(full_size_workload):
+    w = full_size_workload
+    g = lbm.from_workload(w, "FP32")
+    r0, _ = g.read_rho_u()
+    m0 = r0.astype(np.float64).sum()
+    g.step(10)
+    r1, _ = g.read_rho_u()
+    g.close()
+    assert abs(r1.astype(np.float64).sum() - m0) / m0 < 1e-7
