@@ -126,6 +126,27 @@ def dist_setup(n_gpus):
     return world, rank, local
 
 
+def max_over_ranks(ms, device="cuda"):
+    """A step is over when the slowest rank is done: MAX over ranks of a per-rank time (any backend)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_mlups(world, cells_per_rank, steps, ms):
+    """Replicas only: every rank updates its own box; the job's throughput is all ranks'
+    cell updates over the slowest rank's time."""
+    return world * cells_per_rank * steps / (ms * 1e-3) / 1e6
+
+
+def rank_seed(rank):
+    return SEED + rank
+
+
 def run_ours(args):
     import torch
 
@@ -136,18 +157,29 @@ def run_ours(args):
     dist = None
     if world > 1:
         import torch.distributed as dist
-    L, K, W = args.size, args.steps, args.warmup
-    N = L ** 3
+    L, K, W, Q = args.size, args.steps, args.warmup, args.velset
+    nz = 1 if Q == 9 else L
+    N = L * L * nz
     formats = args.formats.split(",")
     peak, peak_src = measured_peak()
 
-    # synthetic input, host side (pinned, for the end-to-end leg) and a device copy
-    w = wl.perturbed_equilibrium(L, L, L, seed=SEED + rank, tau=TAU)
-    rho_h = torch.from_numpy(w.rho).pin_memory()
-    u_h = torch.from_numpy(w.u).pin_memory()
-    rho_d, u_d = rho_h.cuda(), u_h.cuda()
-    rho_out = torch.empty(N, dtype=torch.float32).pin_memory()
-    u_out = torch.empty((3, N), dtype=torch.float32).pin_memory()
+    # synthetic input.  Default: the seeded host arrays of workloads.perturbed_equilibrium, pinned (they are the
+    # end-to-end leg's input) and copied to the device.  --device-init (sweep sizes whose host arrays would be
+    # tens of GB): the same recipe drawn on the device by torch's seeded generator; no end-to-end leg then.
+    host_input = not args.device_init
+    if host_input:
+        w = wl.perturbed_equilibrium(L, L, nz, seed=rank_seed(rank), tau=TAU, velset=Q)
+        rho_h = torch.from_numpy(w.rho).pin_memory()
+        u_h = torch.from_numpy(w.u).pin_memory()
+        rho_d, u_d = rho_h.cuda(), u_h.cuda()
+        rho_out = torch.empty(N, dtype=torch.float32).pin_memory()
+        u_out = torch.empty((3, N), dtype=torch.float32).pin_memory()
+    else:
+        gen = torch.Generator(device="cuda").manual_seed(rank_seed(rank))
+        rho_d = 1.0 + 1e-3 * torch.randn(N, device="cuda", generator=gen)
+        u_d = (0.05 / 3 ** 0.5) * (2.0 * torch.rand((3, N), device="cuda", generator=gen) - 1.0)
+        if Q == 9:
+            u_d[2] = 0.0
 
     sampler = ClockSampler(local)
     if rank == 0:
@@ -160,16 +192,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(ms):
-        if dist is None:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
     results, launches_total = {}, 0
     for name in formats:
-        sim = lbm.Simulation(L, L, L, 19, name, TAU, cells_per_thread=args.cells_per_thread)
+        sim = lbm.Simulation(L, L, nz, Q, name, TAU, cells_per_thread=args.cells_per_thread)
         sim.init(rho_d, u_d)
         sim.step(W)
         barrier()
@@ -187,19 +212,21 @@ def run_ours(args):
         rho_chk, _ = sim.read_rho_u_device()
         assert bool(torch.isfinite(rho_chk).all()), name
         # end to end through the public API with HOST buffers: init (H2D) + K steps + read-out (D2H)
-        barrier()
-        t_e2e = time.perf_counter()
-        sim.init(rho_h.numpy(), u_h.numpy())
-        sim.step(K)
-        sim.read_rho_u(out=(rho_out.numpy(), u_out.numpy()))
-        torch.cuda.synchronize()
-        e2e_ms = max_over_ranks((time.perf_counter() - t_e2e) * 1e3)
-        bpc = lbm.bytes_per_cell(19, name)
-        mlups = world * N * K / (ms * 1e-3) / 1e6
+        e2e_ms = None
+        if host_input:
+            barrier()
+            t_e2e = time.perf_counter()
+            sim.init(rho_h.numpy(), u_h.numpy())
+            sim.step(K)
+            sim.read_rho_u(out=(rho_out.numpy(), u_out.numpy()))
+            torch.cuda.synchronize()
+            e2e_ms = max_over_ranks((time.perf_counter() - t_e2e) * 1e3)
+        bpc = lbm.bytes_per_cell(Q, name)
+        mlups = whole_job_mlups(world, N, K, ms)
         gbs = N * bpc / (ms / K * 1e-3) / 1e9         # per GPU, per launch
         results[name] = {"mlups": round(mlups, 1), "ms_per_step": round(ms / K, 4), "bytes_per_cell": bpc,
                          "hbm_gbs": round(gbs, 1), "frac_of_peak": round(gbs / peak, 4),
-                         "e2e_mlups": round(world * N * K / (e2e_ms * 1e-3) / 1e6, 1), "kernel": sim.kernel_name,
+                         "e2e_mlups": round(whole_job_mlups(world, N, K, e2e_ms), 1) if e2e_ms else None, "kernel": sim.kernel_name,
                          "launches": launches}
         sim.close()
         del sim
@@ -214,16 +241,16 @@ def run_ours(args):
         "metric": METRIC, "value": r["mlups"], "unit": "MLUPs/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"configs[4] bandwidth sweep: D3Q19 BGK periodic cube {L}^3, perturbed equilibrium "
+        "config": {"workload": f"configs[4] bandwidth sweep: D{2 if Q == 9 else 3}Q{Q} BGK periodic {'square' if Q == 9 else 'cube'} {L}^{2 if Q == 9 else 3}, perturbed equilibrium "
                                f"(seed {SEED}), tau {TAU}, headline storage format {head}",
                    "cells": N, "l2_policy": "inputs larger than L2 (two DDF buffers of "
-                                            f"{N * 19 * (4 if head == 'FP32' else 2) / 1e9:.1f} GB each, no flush needed)",
+                                            f"{N * Q * (4 if head == 'FP32' else 2) / 1e9:.1f} GB each, no flush needed)",
                    "parallelism": f"{world} independent replica(s)"},
         "formats": results,
         "speedup_16bit_vs_fp32": (round(results[head]["mlups"] / results["FP32"]["mlups"], 3)
                                   if "FP32" in results and head != "FP32" else None),
         "roofline": {"bound": "hbm", "kernel": r["kernel"], "achieved": r["hbm_gbs"], "peak": peak, "unit": "GB/s",
-                     "frac": r["frac_of_peak"], "traffic": recorded_traffic(head, L), "peak_source": peak_src,
+                     "frac": r["frac_of_peak"], "traffic": recorded_traffic(head, L) if Q == 19 else None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": N * r["bytes_per_cell"]},
         "e2e": {"value": r["e2e_mlups"], "unit": "MLUPs/s", "h2d_bytes_per_step": 16 * N / K,
                 "d2h_bytes_per_step": 16 * N / K,
@@ -293,6 +320,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=512, help="cube edge L")
     ap.add_argument("--formats", default="FP32,FP16S,FP16C,P16_0S,P16_1S,P16_2C")
+    ap.add_argument("--velset", type=int, default=19, choices=[9, 19, 27], help="sweep only; the headline is D3Q19")
+    ap.add_argument("--device-init", action="store_true", help="draw the input on the device (big sweep sizes)")
     ap.add_argument("--cells-per-thread", type=int, default=0, help="0 = library default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

@@ -51,10 +51,11 @@ struct FastDiv {
 
 struct BulkGeom {
     int tiles_per_row;     // ceil(nx / TX)
-    int rows_per_tile;     // RMAX if tiles_per_row == 1, else 1
+    int rows_per_tile;     // rows of a tile: RMAX*TX / nx if a row is one tile (their segments are contiguous), else RMAX
     int ytiles;            // ceil(ny / rows_per_tile)
     int n_tiles;           // tiles_per_row * ytiles * nz  (< 2^31)
     FastDiv by_tpr, by_ytiles;
+    FastDiv by_hw_full, by_hw_last;   // division by half the width of a full tile / of a row's last tile
     long long src_off[27]; // i*N - nx*(c_iy + ny*c_iz): source row of direction i relative to the own row, no wrap
 };
 
@@ -119,9 +120,10 @@ struct BulkShape {
     static constexpr int PAD = 16;                      // halo pad in front of and behind every segment
     static constexpr int MAXB = (227 * 1024 - 2048) / 2;                    // two CTAs per SM
     static constexpr int TABB = PairCodec<F>::TABLE ? 512 * 16 : 0;        // the format's encoder table
-    static constexpr int row_stage(int r) { return Q * (r * TX * ES + 2 * PAD) + r * TX; }
-    static constexpr int RMAX = 2 * row_stage(2) + TABB <= MAXB ? 2 : 1;    // rows per tile (single-tile rows only)
-    static constexpr int ROWB = RMAX * TX * ES + 2 * PAD;                   // one direction of one stage
+    static constexpr int row_stage(int r) { return Q * r * (TX * ES + 2 * PAD) + r * TX; }
+    static constexpr int RMAX = 2 * row_stage(2) + TABB <= MAXB ? 2 : 1;    // full-width rows per tile
+    static constexpr int PITCH = TX * ES + 2 * PAD;                         // row pitch when rows are copied one by one
+    static constexpr int ROWB = RMAX * PITCH;                               // one direction of one stage
     static constexpr int STAGEB = row_stage(RMAX);                          // + the tile's flag bytes
     static constexpr int S = 3 * STAGEB + TABB <= MAXB ? 3 : 2;             // input stages
     static constexpr int TAB_OFF = S * STAGEB;
@@ -184,6 +186,7 @@ struct PullStaged<Q, F, NT, PC, Q> {
 
 struct TileCoord {
     int y, z, x0, w, rows;   // first row, plane, first cell, cells per row (multiple of 16), rows of a tile
+    bool last;               // the last (possibly narrower) tile of its row
 };
 template <int TX>
 __device__ __forceinline__ TileCoord tile_coord(int t, const BulkGeom &g, const Params &p) {
@@ -194,6 +197,7 @@ __device__ __forceinline__ TileCoord tile_coord(int t, const BulkGeom &g, const 
     c.rows = min(g.rows_per_tile, p.ny - c.y);
     c.x0 = xt * TX;
     c.w = min(TX, p.nx - c.x0);
+    c.last = xt == g.tiles_per_row - 1;
     return c;
 }
 
@@ -209,44 +213,49 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     if (lane != 0) return;
     const bool single = g.tiles_per_row == 1;
     const TileCoord c = tile_coord<TX>(t, g, p);
-    const int cells = c.rows * c.w;                                         // rows > 1 only if w == nx
-    if (warp == 0) mbar_arrive_expect_tx(full, (unsigned)(Q * cells * ES + cells + (single ? 0 : n_shift * SH::PAD)));
+    const int cells = c.rows * c.w;
+    // single: the rows of the tile are one contiguous segment per direction (pitch = w elements); else every row
+    // is copied on its own, with its own halo pads (pitch = SH::PITCH bytes)
+    const int pitch = single ? c.w * ES : SH::PITCH;
+    if (warp == 0)
+        mbar_arrive_expect_tx(full, (unsigned)(Q * cells * ES + cells + (single ? 0 : c.rows * n_shift * SH::PAD)));
     const long long own = (long long)p.nx * (c.y + (long long)p.ny * c.z);
     // tiles on a y or z face of the box pull some directions from the opposite face (R2): rare, row by row
     const bool face = c.y == 0 || c.y + c.rows == p.ny || c.z == 0 || c.z == p.nz - 1;
 #pragma unroll 1
     for (int i = warp; i <= Q; i += NW) {
-        if (i == Q) {
-            bulk_g2s(stage + Q * SH::ROWB, p.flags + own + c.x0, (unsigned)cells, full);
+        if (i == Q) {                                                       // flag bytes, rows packed at pitch w
+            if (single) bulk_g2s(stage + Q * SH::ROWB, p.flags + own, (unsigned)cells, full);
+            else
+                for (int r = 0; r < c.rows; ++r)
+                    bulk_g2s(stage + Q * SH::ROWB + r * c.w, p.flags + own + (long long)r * p.nx + c.x0, (unsigned)c.w, full);
             break;
         }
         const int m = Q == 9 ? d2q9_members[i] : i;
         const int cx = c27_table[m][0];
         const unsigned dst = stage + i * SH::ROWB + SH::PAD;
-        const T *src_row;
-        if (!face) {
-            src_row = A + own + g.src_off[i];
-            bulk_g2s(dst, src_row + c.x0, (unsigned)(cells * ES), full);
-        } else {
-            const int cy = c27_table[m][1], cz = c27_table[m][2];
-            int zs = c.z - cz;
-            zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
-            src_row = nullptr;
-#pragma unroll 1
-            for (int r = 0; r < c.rows; ++r) {
-                int ys = c.y + r - cy;
-                ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
-                src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
-                bulk_g2s(dst + r * c.w * ES, src_row + c.x0, (unsigned)(c.w * ES), full);
-            }
+        if (single && !face) {
+            bulk_g2s(dst, A + own + g.src_off[i], (unsigned)(cells * ES), full);
+            continue;
         }
-        if (!single && cx != 0) {                                           // multi-tile rows: rows == 1
-            if (cx > 0) {                                                   // element x0 - 1: the chunk before x0
-                const int xs = (c.x0 == 0 ? p.nx : c.x0) - SH::HALO_ELEMS;
-                bulk_g2s(dst - SH::PAD, src_row + xs, SH::PAD, full);
-            } else {                                                        // element x0 + w: the chunk after the tile
-                const int xs = c.x0 + c.w == p.nx ? 0 : c.x0 + c.w;
-                bulk_g2s(dst + c.w * ES, src_row + xs, SH::PAD, full);
+        const int cy = c27_table[m][1], cz = c27_table[m][2];
+        int zs = c.z - cz;
+        zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
+#pragma unroll 1
+        for (int r = 0; r < c.rows; ++r) {
+            int ys = c.y + r - cy;
+            ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
+            const T *src_row = A + (long long)i * p.N + (long long)p.nx * (ys + (long long)p.ny * zs);
+            const unsigned d = dst + r * pitch;
+            bulk_g2s(d, src_row + c.x0, (unsigned)(c.w * ES), full);
+            if (!single && cx != 0) {
+                if (cx > 0) {                                               // element x0 - 1: the chunk before x0
+                    const int xs = (c.x0 == 0 ? p.nx : c.x0) - SH::HALO_ELEMS;
+                    bulk_g2s(d - SH::PAD, src_row + xs, SH::PAD, full);
+                } else {                                                    // element x0 + w: the chunk after the tile
+                    const int xs = c.x0 + c.w == p.nx ? 0 : c.x0 + c.w;
+                    bulk_g2s(d + c.w * ES, src_row + xs, SH::PAD, full);
+                }
             }
         }
     }
@@ -293,21 +302,25 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
         if (t < g.n_tiles) issue_tile_loads<Q, F, NT>(A, p, g, (int)t, smem_base + s * SH::STAGEB, bar_full + s * 8, warp, lane);
     }
 
-    const int xl = 2 * tid;
     int k = 0;
     for (int t = blockIdx.x; t < g.n_tiles; t += stride, ++k) {
         const int s = k % S;
         const unsigned ph = (unsigned)(k / S) & 1u;
         const TileCoord c = tile_coord<TX>(t, g, p);
-        const int w = c.w;
-        const bool active = xl < w;
+        const int w = c.w, hw = w >> 1;
         const char *stage = smem + s * SH::STAGEB;
-        const int el = xl - 1 + ((single && xl == 0) ? w : 0);                  // element "xl - 1" of a row
-        const int er = xl + 2 - ((single && xl + 2 == w) ? w : 0);              // element "xl + 2" of a row
+        const int pitch = single ? w * ES : SH::PITCH;
+        const int pairs = c.rows * hw;                                          // cell pairs of the tile
+        const FastDiv by_hw = c.last ? g.by_hw_last : g.by_hw_full;
 
         mbar_wait(bar_full + s * 8, ph);
 #pragma unroll 1
-        for (int r = 0; r < c.rows; ++r) {
+        for (int it = 0, fp = tid; it * NT < pairs; ++it, fp += NT) {           // same trip count for every thread
+            const bool active = fp < pairs;
+            const int r = hw == NT ? it : by_hw.div(fp);                        // row of the tile holding this cell pair
+            const int xl = 2 * (fp - r * hw);
+            const int el = xl - 1 + ((single && xl == 0) ? w : 0);              // element "xl - 1" of the row
+            const int er = xl + 2 - ((single && xl + 2 == w) ? w : 0);          // element "xl + 2" of the row
             const int y = c.y + r, z = c.z;
             const long long own = (long long)p.nx * (y + (long long)p.ny * z) + c.x0 + xl;   // the thread's first cell
             unsigned fl = 0;
@@ -315,7 +328,7 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             const bool fast = active && fl == 0;
             float f[2][Q];
             unsigned acc = 0;
-            const char *base = stage + SH::PAD + r * w * ES;
+            const char *base = stage + SH::PAD + r * pitch;
             if (fast) PullStaged<Q, F, NT, PC, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
             // codes outside the fast decoders' domain (posits: a regime of ones): this pair goes through Codec<F>
             const bool exact = PC::CHECK != 0 && ((acc | (acc >> 16)) & PC::CHECK) != 0;
@@ -323,7 +336,7 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
                 unsigned dummy = 0;
                 PullStaged<Q, F, NT, PairCodec<-1 - F>, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, dummy);
             }
-            if (r + 1 == c.rows) {                                              // the warp has its values in registers:
+            if ((it + 1) * NT >= pairs) {                                       // last trip: the warp has its values in registers,
                 __syncwarp();                                                   // the stage may be refilled
                 if (lane == 0) mbar_arrive(bar_empty + s * 8);
             }
