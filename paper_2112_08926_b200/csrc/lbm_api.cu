@@ -98,10 +98,12 @@ int ensure_ddf(lbm *h) {
     return LBM_OK;
 }
 
-// Kernel variant.  Automatic choice: the shared-memory-staged kernel (lbm_bulk.cuh) for every 16-bit format
-// when rows are 16-cell aligned and at least half a tile long -- it is what lifts the 16-bit formats out of
-// the issue bound; FP32 storage stays on the per-thread kernel, which already runs at
-// the HBM roofline.  Per-thread kernel: the widest of {2, 1} cells per thread that divides nx.
+// Kernel variant.  Automatic choice, from the bandwidth sweep recorded in DESIGN.md section 6:
+//   * FP32 storage: the per-thread kernel (it runs at the HBM roofline);
+//   * 16-bit formats, D3Q19 / D3Q27, rows 16-cell aligned and >= 64 cells, box >= 2^20 cells: the
+//     shared-memory-staged kernel (lbm_bulk.cuh), which lifts them out of the issue bound;
+//   * D2Q9 (9 streams: the staged kernel's per-tile bookkeeping does not pay) and small boxes (L2-resident,
+//     launch-bound): the per-thread kernel, 4 cells per thread for D2Q9, else 2.
 int pick_variant(const lbm *h) {
     int want = h->V_request;
     if (want == 0) {
@@ -110,8 +112,8 @@ int pick_variant(const lbm *h) {
     }
     const bool bulk_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->bulk_tile_cells() - 1) / h->ops->bulk_tile_cells()) * h->ny * h->nz <= 0x7FFFFFFFLL;
     if (want == LBM_VARIANT_BULK && bulk_ok) return LBM_VARIANT_BULK;
-    if (want == 0 && bulk_ok && h->fmt != LBM_FP32 && 2 * h->nx >= h->ops->bulk_tile_cells()) return LBM_VARIANT_BULK;
-    if (want != 1 && want != 2 && want != 4) want = 2;
+    if (want == 0 && bulk_ok && h->fmt != LBM_FP32 && h->q != LBM_D2Q9 && h->nx >= 64 && h->N >= (1LL << 20)) return LBM_VARIANT_BULK;
+    if (want != 1 && want != 2 && want != 4) want = (h->q == LBM_D2Q9 && h->fmt != LBM_FP32) ? 4 : 2;
     while (want > 1 && h->nx % want != 0) want >>= 1;
     return want;
 }

@@ -190,7 +190,7 @@ def test_bulk_variant_taylor_green_and_cavity(name, variant, tag):
 
 
 def test_automatic_variant_choice():
-    w = wl.perturbed_equilibrium(256, 2, 2, seed=2)
+    w = wl.perturbed_equilibrium(256, 64, 64, seed=2)
     g16 = lbm.from_workload(w, "FP16S")
     g32 = lbm.from_workload(w, "FP32")
     assert "bulk" in g16.kernel_name and "bulk" not in g32.kernel_name
