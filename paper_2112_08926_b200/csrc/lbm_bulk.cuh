@@ -50,7 +50,8 @@ struct FastDiv {
 };
 
 struct BulkGeom {
-    int tiles_per_row;     // ceil(nx / TX)
+    int tile_w;            // cells of a full tile row: nx if a whole row fits a stage (nx <= RMAX*TX), else TX
+    int tiles_per_row;     // ceil(nx / tile_w)
     int rows_per_tile;     // rows of a tile: RMAX*TX / nx if a row is one tile (their segments are contiguous), else RMAX
     int ytiles;            // ceil(ny / rows_per_tile)
     int n_tiles;           // tiles_per_row * ytiles * nz  (< 2^31)
@@ -177,15 +178,14 @@ struct TileCoord {
     int y, z, x0, w, rows;   // first row, plane, first cell, cells per row (multiple of 16), rows of a tile
     bool last;               // the last (possibly narrower) tile of its row
 };
-template <int TX>
 __device__ __forceinline__ TileCoord tile_coord(int t, const BulkGeom &g, const Params &p) {
     TileCoord c;
     const int rt = g.by_tpr.div(t), xt = t - rt * g.tiles_per_row;
     c.z = g.by_ytiles.div(rt);
     c.y = (rt - c.z * g.ytiles) * g.rows_per_tile;
     c.rows = min(g.rows_per_tile, p.ny - c.y);
-    c.x0 = xt * TX;
-    c.w = min(TX, p.nx - c.x0);
+    c.x0 = xt * g.tile_w;
+    c.w = min(g.tile_w, p.nx - c.x0);
     c.last = xt == g.tiles_per_row - 1;
     return c;
 }
@@ -201,7 +201,7 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     constexpr int n_shift = (Q == 9 ? 6 : Q == 19 ? 10 : 18);               // directions with c_x != 0
     if (lane != 0) return;
     const bool single = g.tiles_per_row == 1;
-    const TileCoord c = tile_coord<TX>(t, g, p);
+    const TileCoord c = tile_coord(t, g, p);
     const int cells = c.rows * c.w;
     // single: the rows of the tile are one contiguous segment per direction (pitch = w elements); else every row
     // is copied on its own, with its own halo pads (pitch = SH::PITCH bytes)
@@ -295,7 +295,7 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
     for (int t = blockIdx.x; t < g.n_tiles; t += stride, ++k) {
         const int s = k % S;
         const unsigned ph = (unsigned)(k / S) & 1u;
-        const TileCoord c = tile_coord<TX>(t, g, p);
+        const TileCoord c = tile_coord(t, g, p);
         const int w = c.w, hw = w >> 1;
         const char *stage = smem + s * SH::STAGEB;
         const int pitch = single ? w * ES : SH::PITCH;

@@ -40,10 +40,11 @@ constexpr int BULK_NT = 256;
 BulkGeom bulk_geom(const Params &p, long long *tiles) {
     typedef BulkShape<Q, F, BULK_NT> SH;
     BulkGeom g;
-    g.tiles_per_row = (p.nx + SH::TX - 1) / SH::TX;
+    g.tile_w = p.nx <= SH::RMAX * SH::TX ? p.nx : SH::TX;
+    g.tiles_per_row = (p.nx + g.tile_w - 1) / g.tile_w;
     g.rows_per_tile = g.tiles_per_row == 1 ? SH::RMAX * SH::TX / p.nx : SH::RMAX;
-    const int w_full = p.nx < SH::TX ? p.nx : SH::TX, w_last = p.nx - (g.tiles_per_row - 1) * SH::TX;
-    g.by_hw_full = FastDiv::make(w_full / 2);
+    const int w_last = p.nx - (g.tiles_per_row - 1) * g.tile_w;
+    g.by_hw_full = FastDiv::make(g.tile_w / 2);
     g.by_hw_last = FastDiv::make(w_last / 2);
     g.ytiles = (p.ny + g.rows_per_tile - 1) / g.rows_per_tile;
     *tiles = (long long)g.tiles_per_row * g.ytiles * p.nz;

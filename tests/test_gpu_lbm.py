@@ -149,7 +149,8 @@ def test_mass_conservation_fp32():
 # ---- the shared-memory-staged kernel (lbm_bulk.cuh): same results, bit for bit ------------------------
 # shapes: one tile per row (x wraps inside the segment), several tiles per row with a ragged last tile (halo
 # copies, wrap at the row ends), the smallest legal row (16 cells), 2-D
-BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16, 4, 5)), (19, (512, 2, 1)),
+BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16, 4, 5)), (19, (512, 2, 1)), (19, (1024, 3, 2)),
+               (19, (2064, 2, 1)),
                (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1))]
 
 
@@ -166,7 +167,8 @@ def test_bulk_variant_periodic(q, shape, name, variant, tag):
     assert_parity(osim, gsim, name)
 
 
-@pytest.mark.parametrize("q,shape", [(19, (48, 7, 5)), (19, (544, 3, 3)), (27, (32, 6, 5)), (9, (64, 11, 1))])
+@pytest.mark.parametrize("q,shape", [(19, (48, 7, 5)), (19, (544, 3, 3)), (19, (1040, 3, 2)), (27, (32, 6, 5)), (27, (1072, 2, 2)),
+                                     (9, (64, 11, 1))])
 @pytest.mark.parametrize("name", ALL_FORMATS)
 @pytest.mark.parametrize("variant,tag", STAGED)
 def test_bulk_variant_walls_moving_walls_force(q, shape, name, variant, tag):
