@@ -23,6 +23,8 @@
 //   - exponent bits cut off by a long regime count as 0; if one of P16_2C's two bits is left it is the
 //     HIGH bit (posit convention), which keeps the value table strictly monotone.
 //
+// PARITY UNPINNED: the class-B corners of rule U (P16_1S outside 2^-33 <= |x| < 2^19, P16_2C below 2^-51 and in
+// [2 - 2^-13, 2)), where the paper's listing is not a nearest-value converter (R14).
 // Pins (tests/test_oracle_codecs.py): Table 2 constants, strict monotonicity, exhaustive round trip,
 // numpy float16 for FP16/FP16S, and an independent transcription of Listing 1 kept in tests/.
 #include "oracle.h"

@@ -14,6 +14,9 @@
 //   R8  f_i^B(x) = fma(1-omega, f_i^temp, omega f_i^eq)                        eq (28)
 //   R10 Guo forcing source term (named at PAPER.md:233, formula: DESIGN.md R10)
 // with load()/store() = the codecs of codecs.cpp applied at every read and write.
+// PARITY UNPINNED (no external pin exists; fixed by DESIGN.md section 3 only): the operation order of R5 / R10, the
+// pre-computation grouping of R7, rho_w = 1 in R9, writing both buffers in R11, R12 as the definition of the
+// read-out, the D2Q9 / D3Q27 direction numbering.  Everything else is pinned by tests/test_oracle_lbm.py.
 // Arithmetic type T = float reproduces the paper's FP32 arithmetic (parity runs); T = double is used
 // for the analytic pins (tests/test_oracle_lbm.py).  Everything is written as plain loops over the
 // velocity-set table; operation order is the one stated in DESIGN.md section 3.
