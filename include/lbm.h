@@ -46,7 +46,12 @@ enum {
     LBM_P16_2C = 5, /* one-sided regime, 2 exponent bits, unscaled */
     LBM_FP16 = 6    /* plain IEEE binary16 (Table 2 row 139)                          */
 };
-enum { LBM_FLAG_WALL = 0x01 };
+/* LBM_FLAG_WALL: halfway bounce-back wall cell (TYPE_W), optionally moving (its u).
+ * LBM_FLAG_EQ:   equilibrium boundary cell (TYPE_E; "equilibrium boundaries"; R15): it keeps
+ *                the DDFs lbm_init gave it -- the shifted equilibrium of its rho, u -- for ever; its neighbours pull
+ *                from it as from a fluid cell (inflow / outflow / free-stream perimeter).
+ * Neither kind of cell is written by lbm_step; lbm_read_rho_u returns for them the fields given to lbm_init. */
+enum { LBM_FLAG_WALL = 0x01, LBM_FLAG_EQ = 0x02 };
 enum {
     LBM_OK = 0,
     LBM_E_INVAL = -1,       /* bad argument                                   */
@@ -80,7 +85,7 @@ enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16 };
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_cells_per_thread(lbm_t *h, int v);
 
-/* Set the cell flags.  flags: HOST pointer, N bytes, copied.  Only LBM_FLAG_WALL may be set
+/* Set the cell flags.  flags: HOST pointer, N bytes, copied.  Only LBM_FLAG_WALL or LBM_FLAG_EQ may be set (not both on one cell)
  * (else LBM_E_INVAL).  Must precede lbm_init (LBM_E_STATE otherwise).  Synchronises the stream. */
 int lbm_set_flags(lbm_t *h, const unsigned char *flags);
 

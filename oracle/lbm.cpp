@@ -13,6 +13,7 @@
 //   R7  shifted equilibrium "exactly as presented" in eq (3), 3 FMAs
 //   R8  f_i^B(x) = fma(1-omega, f_i^temp, omega f_i^eq)                        eq (28)
 //   R10 Guo forcing source term (named at PAPER.md:233, formula: DESIGN.md R10)
+//   R15 equilibrium boundary cells (named at PAPER.md:322): never updated, they keep f^eq(rho0, u0) from init
 // with load()/store() = the codecs of codecs.cpp applied at every read and write.
 // PARITY UNPINNED (no external pin exists; fixed by DESIGN.md section 3 only): the operation order of R5 / R10, the
 // pre-computation grouping of R7, rho_w = 1 in R9, writing both buffers in R11, R12 as the definition of the
@@ -228,7 +229,7 @@ void step_t(orc_sim *s) {
         for (int y = 0; y < ny; ++y)
             for (int x = 0; x < nx; ++x) {
                 const long n = x + (long)nx * (y + (long)ny * z);
-                if (s->flags[n] & ORC_FLAG_WALL) continue;
+                if (s->flags[n] & (ORC_FLAG_WALL | ORC_FLAG_EQ)) continue;   // PAPER.md:1017; R15: E cells keep feq(rho0, u0)
                 T fh[27];
                 fh[0] = load<T>(s, A, 0, n);
                 for (int i = 1; i < q; ++i) {
@@ -284,7 +285,7 @@ void read_t(orc_sim *s, T *rho_out, T *u_out) {
     const T F[3] = {(T)s->force[0], (T)s->force[1], (T)s->force[2]};
 #pragma omp parallel for schedule(static)
     for (long n = 0; n < s->N; ++n) {
-        if (s->flags[n] & ORC_FLAG_WALL) {
+        if (s->flags[n] & (ORC_FLAG_WALL | ORC_FLAG_EQ)) {
             const bool dbl = s->arith == ORC_ARITH_F64 && !s->rho0d.empty();
             if (rho_out) rho_out[n] = dbl ? (T)s->rho0d[n] : (T)s->rho0[n];
             if (u_out)

@@ -22,7 +22,7 @@ extern "C" {
 enum { ORC_FP32 = 0, ORC_FP16S = 1, ORC_FP16C = 2, ORC_P16_0S = 3, ORC_P16_1S = 4, ORC_P16_2C = 5,
        ORC_FP16 = 6, ORC_FP64 = 7 /* oracle only: raw doubles, needs arith = 1 */ };
 enum { ORC_ARITH_F32 = 0, ORC_ARITH_F64 = 1 };
-enum { ORC_FLAG_WALL = 0x01 };
+enum { ORC_FLAG_WALL = 0x01, ORC_FLAG_EQ = 0x02 /* equilibrium boundary cell: keeps its init DDFs (R15) */ };
 
 /* ---- codecs (16-bit formats only, fmt in 1..6) ------------------------------------------------ */
 /* unscaled table value V(mag) of the 15-bit magnitude field, as a double (Inf/NaN for FP16 e=31) */

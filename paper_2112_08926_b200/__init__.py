@@ -27,7 +27,7 @@ D2Q9, D3Q19, D3Q27 = 9, 19, 27
 BGK, TRT = 0, 1
 FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C": 5, "FP16": 6}
 FORMAT_NAMES = {v: k for k, v in FORMATS.items()}
-FLAG_WALL = 0x01
+FLAG_WALL, FLAG_EQ = 0x01, 0x02
 VARIANT_AUTO, VARIANT_BULK = 0, 16
 OK, E_INVAL, E_UNSUPPORTED, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 

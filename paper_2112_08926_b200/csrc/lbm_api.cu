@@ -219,7 +219,8 @@ int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
     if (h->inited) return fail(LBM_E_STATE, "lbm_set_flags: must be called before lbm_init");
     bool walls = false;
     for (long long n = 0; n < h->N; ++n) {
-        if (flags[n] & ~LBM_FLAG_WALL) return fail(LBM_E_INVAL, "lbm_set_flags: unknown flag bit set");
+        if (flags[n] & ~(LBM_FLAG_WALL | LBM_FLAG_EQ)) return fail(LBM_E_INVAL, "lbm_set_flags: unknown flag bit set");
+        if (flags[n] == (LBM_FLAG_WALL | LBM_FLAG_EQ)) return fail(LBM_E_INVAL, "lbm_set_flags: a cell cannot be wall and equilibrium boundary");
         walls |= flags[n] != 0;
     }
     h->has_walls = walls;

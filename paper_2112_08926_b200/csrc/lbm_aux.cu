@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(256) mark_near_kernel(const unsigned char *__r
     const int y = blockIdx.y, z = blockIdx.z;
     if (x >= nx) return;
     const long long n = x + (long long)nx * (y + (long long)ny * z);
-    unsigned fl = in[n] & FLAG_WALL;
+    unsigned fl = in[n] & FLAG_FIXED;
     if (!fl) {
         unsigned near = 0;
 #pragma unroll

@@ -359,7 +359,7 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
                         for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
 #pragma unroll 1
                     for (int j = 0; j < 2; ++j) {
-                        if ((fl >> (8 * j)) & FLAG_WALL) continue;              // wall cells are not updated
+                        if ((fl >> (8 * j)) & FLAG_FIXED) continue;             // wall (and E) cells are not updated
                         const int x = c.x0 + xl + j;
                         const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
                         float gq[Q];

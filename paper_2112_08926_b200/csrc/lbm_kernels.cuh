@@ -220,7 +220,7 @@ stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F
         // ---- a wall cell or a wall neighbour in this thread's cells: cell by cell ------------------
 #pragma unroll 1
         for (int j = 0; j < V; ++j) {
-            if ((any >> (8 * j)) & FLAG_WALL) continue;
+            if ((any >> (8 * j)) & FLAG_FIXED) continue;                   // PAPER.md:1017; R15
             const int x = x0 + j;
             const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
             float g[Q];
@@ -261,7 +261,7 @@ read_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, flo
     const long long N = p.N;
     for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
         float rho, j[3], u[3];
-        if (__ldg(p.flags + n) & FLAG_WALL) {
+        if (__ldg(p.flags + n) & FLAG_FIXED) {
             rho = __ldg(p.rho0 + n);
 #pragma unroll
             for (int a = 0; a < 3; ++a) u[a] = __ldg(p.u0 + a * N + n);

@@ -260,3 +260,51 @@ def test_full_size_mass_conservation(full_size_workload):
     r1, _ = g.read_rho_u()
     g.close()
     assert abs(r1.astype(np.float64).sum() - m0) / m0 < 1e-7
+
+
+# ---- equilibrium boundary cells (LBM_FLAG_EQ, R15) and the Karman set-up of BASELINE configs[3] ----
+EQ_CASES = [(q, shape, v) for q, shape in [(19, (24, 9, 7)), (19, (272, 6, 5)), (27, (32, 7, 5)), (9, (48, 13, 1))]
+            for v in (1, 2, lbm.VARIANT_BULK) if v != lbm.VARIANT_BULK or shape[0] % 16 == 0]
+
+
+@pytest.mark.parametrize("q,shape,variant", EQ_CASES)
+@pytest.mark.parametrize("name", ALL_FORMATS)
+def test_equilibrium_boundary_cells(q, shape, name, variant):
+    w = wl.perturbed_equilibrium(*shape, seed=31, velset=q, tau=0.75)
+    w = wl.random_walls(w, 0.08, seed=33, moving_fraction=0.5)
+    w = wl.equilibrium_rim(w, rho_e=1.005)
+    w.force = (1e-5, 0.0, 0.0)
+    osim, gsim = run_pair(w, name, 20, variant=variant)
+    assert_parity(osim, gsim, name)
+
+
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "FP16C", "P16_2C"])
+def test_karman_config4_small(name):
+    """configs[3] at oracle size: cylinder of wall cells, equilibrium perimeter, asymmetric start; the probe signal
+    behind the cylinder must be the oracle's, bit for bit, at every sampled step."""
+    w = wl.karman_vortex_street(128, 48, 8, radius=3.0, u_in=0.05)
+    osim = oracle.from_workload(w, FORMATS[name])
+    gsim = lbm.from_workload(w, name)
+    px, py, pz = w.meta["probe"]
+    n = px + w.nx * (py + w.ny * pz)
+    for _ in range(6):
+        osim.step(200)
+        gsim.step(200)
+        orho, ou = osim.read_rho_u()
+        grho, gu = gsim.read_rho_u()
+        assert gu[1, n].view(np.uint32) == ou[1, n].view(np.uint32)
+    assert_parity(osim, gsim, name)
+    assert np.abs(ou[1]).max() > 1e-4            # the wake is not symmetric: shedding has started
+
+
+def test_flag_validation_with_equilibrium_bit():
+    s = lbm.Simulation(8, 4, 4, 19, "FP32", 0.6)
+    fl = np.zeros(128, np.uint8)
+    fl[3] = lbm.FLAG_WALL | lbm.FLAG_EQ
+    with pytest.raises(lbm.LbmError):
+        s.set_flags(fl)
+    fl[3] = 4
+    with pytest.raises(lbm.LbmError):
+        s.set_flags(fl)
+    fl[3] = lbm.FLAG_EQ
+    s.set_flags(fl)

@@ -238,6 +238,7 @@ def _reference_push_unshifted(w, steps):
     rho = w.rho.astype(np.float64).reshape(shape)
     u = w.u.astype(np.float64).reshape((3,) + shape)
     wall = (w.flags.reshape(shape) & wl.FLAG_WALL) != 0
+    eqb = (w.flags.reshape(shape) & wl.FLAG_EQ) != 0                 # equilibrium boundary cells (R15)
     F = np.array(w.force, np.float64)
     omega = 1.0 / w.tau
 
@@ -250,6 +251,7 @@ def _reference_push_unshifted(w, steps):
         return out
 
     f = feq(rho, u)                                                  # post-"collision" state at t = 0
+    f_imposed = f.copy()
     uw = np.where(wall[None], u, 0.0)
     cs = 1 / math.sqrt(3)
     for _ in range(steps):
@@ -275,11 +277,12 @@ def _reference_push_unshifted(w, steps):
                 uF = un[0] * F[0] + un[1] * F[1] + un[2] * F[2]
                 new[i] += (1 - 0.5 * omega) * wts[i] * (3 * (cF - uF) + 9 * cu * cF)
         f = np.where(wall[None], f, new)                             # wall cells are never updated
+        f = np.where(eqb[None], f_imposed, f)                        # E cells are reset to their imposed equilibrium
     rho_o = f.sum(0)
     j = np.einsum("ia,i...->a...", c.astype(np.float64), f)
     u_o = (j - 0.5 * F[:, None, None, None]) / rho_o
-    rho_o = np.where(wall, rho, rho_o)
-    u_o = np.where(wall[None], u, u_o)
+    rho_o = np.where(wall | eqb, rho, rho_o)
+    u_o = np.where((wall | eqb)[None], u, u_o)
     return rho_o.reshape(-1), u_o.reshape(3, -1)
 
 
@@ -300,6 +303,42 @@ def test_against_push_unshifted_reference(q, shape, force):
     rref, uref = _reference_push_unshifted(w, steps)
     assert np.abs(rho - rref).max() < 5e-14
     assert np.abs(u - uref).max() < 5e-14
+
+
+@pytest.mark.parametrize("q,shape", [(19, (7, 6, 5)), (27, (6, 6, 4)), (9, (8, 7, 1))])
+def test_equilibrium_boundaries_against_push_reference(q, shape):
+    """R15: equilibrium boundary cells, walls and moving walls together, vs the second implementation (which
+    resets E cells to their imposed equilibrium after every step)."""
+    w = wl.perturbed_equilibrium(*shape, seed=13, velset=q, rho_sigma=1e-2, tau=0.8)
+    w = wl.random_walls(w, 0.1, seed=6, moving_fraction=0.5)
+    w = wl.equilibrium_rim(w, rho_e=1.01)
+    s = sim64(w)
+    s.step(9)
+    rho, u = s.read_rho_u(f64=True)
+    rref, uref = _reference_push_unshifted(w, 9)
+    assert np.abs(rho - rref).max() < 5e-14
+    assert np.abs(u - uref).max() < 5e-14
+
+
+def test_equilibrium_perimeter_drives_the_box_to_its_velocity():
+    """A box whose x / y perimeter imposes (rho, u) by equilibrium cells and whose fluid starts at
+    rest ends in the uniform state (rho, u): E cells feed the flow (they are not walls) and uniform flow is the
+    fixed point; started in that state it stays there to rounding."""
+    ue = (0.04, -0.02, 0.0)
+    w = wl.perturbed_equilibrium(10, 9, 2, seed=3, rho_sigma=0.0, u_abs_max=0.0, tau=0.9)
+    w = wl.equilibrium_rim(w, rho_e=1.0, u_e=ue)
+    fluid = w.flags == 0
+    s = sim64(w)
+    s.step(3000)
+    rho, u = s.read_rho_u(f64=True)
+    for a in range(3):
+        assert np.abs(u[a][fluid] - np.float32(ue[a])).max() < 1e-9
+    assert np.abs(rho[fluid] - 1.0).max() < 1e-9
+    w.u = np.tile(np.array(ue, np.float32)[:, None], (1, w.n_cells))
+    s = sim64(w)
+    s.step(50)
+    rho, u = s.read_rho_u(f64=True)
+    assert np.abs(u[0] - np.float32(ue[0])).max() < 1e-14 and np.abs(rho - 1.0).max() < 1e-14
 
 
 def test_axis_permutation_symmetry():

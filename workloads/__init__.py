@@ -20,6 +20,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 FLAG_WALL = 0x01
+FLAG_EQ = 0x02      # equilibrium boundary cell (TYPE_E)
 
 # velocity-set / collision / storage-format ids of include/lbm.h (interface constants, not arithmetic)
 D2Q9, D3Q19, D3Q27 = 9, 19, 27
@@ -159,6 +160,51 @@ def random_walls(w: Workload, fraction: float, seed: int = 7, moving_fraction: f
         w.u = np.where(wall[None, :], np.float32(0), w.u).astype(np.float32)
     return w
 
+
+
+def karman_vortex_street(nx: int = 256, ny: int = 64, nz: int = 16, radius: float = 4.0, x_cyl: int | None = None,
+                         u_in: float = 0.05, tau: float | None = None, Re: float = 200.0, velset: int = D3Q19) -> Workload:
+    """BASELINE.json configs[3] (shape of PAPER.md:320-336): a channel with a z-spanning cylinder of wall cells at
+    (x_cyl, ny/2), flow along +x.  The x = 0, x = nx-1, y = 0 and y = ny-1 planes are equilibrium boundary cells
+    holding rho = 1, u = (u_in, 0, 0) (the paper enforces the velocity on the box perimeter with equilibrium
+    boundaries); z is periodic.  Asymmetric start as in PAPER.md:330: the fluid moves with u_in in
+    one half of the box (y < ny/2) and rests in the other, so that shedding starts at once in every number format.
+    tau defaults to the value Re = 2 R u_in / nu gives."""
+    if x_cyl is None:
+        x_cyl = nx // 4
+    if tau is None:
+        nu = 2.0 * radius * u_in / Re
+        tau = 3.0 * nu + 0.5
+    nzz = 1 if velset == D2Q9 else nz
+    N = nx * ny * nzz
+    z, y, x = np.meshgrid(np.arange(nzz), np.arange(ny), np.arange(nx), indexing="ij")
+    flags = np.zeros((nzz, ny, nx), np.uint8)
+    flags[(x - x_cyl) ** 2 + (y - ny // 2) ** 2 <= radius * radius] = FLAG_WALL
+    rim = (x == 0) | (x == nx - 1) | (y == 0) | (y == ny - 1)
+    flags[rim] = FLAG_EQ
+    ux = np.where(rim | (y < ny // 2), u_in, 0.0)
+    ux[flags == FLAG_WALL] = 0.0
+    u = _pack(ux.reshape(-1), np.zeros(N), np.zeros(N))
+    return Workload("karman_vortex_street", nx, ny, nzz, velset, float(tau), np.ones(N, np.float32), u,
+                    flags.reshape(-1), steps=100000,
+                    meta={"u_in": u_in, "radius": radius, "x_cyl": x_cyl, "probe": (nx // 2, ny // 2, nzz // 2)})
+
+
+def equilibrium_rim(w: Workload, rho_e: float = 1.0, u_e=(0.03, -0.01, 0.02)) -> Workload:
+    """Test helper: turn the x and y faces of a workload into equilibrium boundary cells holding (rho_e, u_e)."""
+    f = w.flags.reshape(w.nz, w.ny, w.nx).copy()
+    rim = np.zeros_like(f, bool)
+    rim[:, :, 0] = rim[:, :, -1] = True
+    rim[:, 0, :] = rim[:, -1, :] = True
+    f[rim] = FLAG_EQ
+    w.flags = f.reshape(-1)
+    r = rim.reshape(-1)
+    w.rho = np.where(r, np.float32(rho_e), w.rho).astype(np.float32)
+    ue = np.array(u_e, np.float32)
+    if w.velset == D2Q9:
+        ue[2] = 0.0
+    w.u = np.where(r[None, :], ue[:, None], w.u).astype(np.float32)
+    return w
 
 def codec_probe_inputs(seed: int = 1, per_binade: int = 4096) -> np.ndarray:
     """float32 inputs for encoder parity: every binade 2^-70 .. 2^24 sampled `per_binade` times with
