@@ -107,6 +107,10 @@ int lbm_step(lbm_t *h, int n);
 int lbm_read_rho_u(lbm_t *h, float *rho, float *u);
 int lbm_read_rho_u_device(lbm_t *h, float *rho_dev, float *u_dev);
 
+/* The same read-out at `count` selected cells (probes of a long run): cells = HOST array of cell indices n,
+ * rho = HOST count floats, u = HOST 3*count floats (ux of all probes | uy | uz).  Synchronises. */
+int lbm_read_rho_u_at(lbm_t *h, const long long *cells, int count, float *rho, float *u);
+
 /* Copy direction i (0 <= i < q) of the current DDF buffer, as stored (N elements of 2 or 4 bytes),
  * to a HOST pointer.  Synchronises.  For bit-level parity tests. */
 int lbm_read_ddf(lbm_t *h, int i, void *out);

@@ -44,6 +44,7 @@ SYMBOLS = {
     "lbm_step": (_i, [_p, _i]),
     "lbm_read_rho_u": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_device": (_i, [_p, _p, _p]),
+    "lbm_read_rho_u_at": (_i, [_p, _p, _i, _p, _p]),
     "lbm_read_ddf": (_i, [_p, _i, _p]),
     "lbm_sync": (_i, [_p]),
     "lbm_steps_done": (_ll, [_p]),
@@ -219,6 +220,14 @@ class Simulation:
         rho = torch.empty(self.N, dtype=torch.float32, device="cuda")
         u = torch.empty((3, self.N), dtype=torch.float32, device="cuda")
         _check(lib().lbm_read_rho_u_device(self._h, rho.data_ptr(), u.data_ptr()))
+        return rho, u
+
+    def read_rho_u_at(self, cells):
+        """Read-out at selected cells: returns (rho [k], u [3, k])."""
+        cells = np.ascontiguousarray(cells, dtype=np.int64).reshape(-1)
+        rho = np.empty(cells.size, np.float32)
+        u = np.empty((3, cells.size), np.float32)
+        _check(lib().lbm_read_rho_u_at(self._h, _np_ptr(cells), cells.size, _np_ptr(rho), _np_ptr(u)))
         return rho, u
 
     def read_ddf(self, i: int) -> np.ndarray:

@@ -327,6 +327,28 @@ int lbm_read_rho_u(lbm_t *h, float *rho, float *u) {
     return LBM_OK;
 }
 
+int lbm_read_rho_u_at(lbm_t *h, const long long *cells, int count, float *rho, float *u) {
+    if (int rc = enter(h)) return rc;
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u_at: call lbm_init first");
+    if (count < 0 || (count > 0 && (!cells || !rho || !u))) return fail(LBM_E_INVAL, "lbm_read_rho_u_at: bad arguments");
+    if (count == 0) return LBM_OK;
+    for (int k = 0; k < count; ++k)
+        if (cells[k] < 0 || cells[k] >= h->N) return fail(LBM_E_INVAL, "lbm_read_rho_u_at: cell index out of range");
+    char *d = nullptr;
+    const size_t cb = (size_t)count * 8, fb = (size_t)count * 16;
+    LBM_CUDA_TRY(cudaMalloc((void **)&d, cb + fb));
+    float *df = (float *)(d + cb);
+    cudaError_t e = cudaMemcpyAsync(d, cells, cb, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = h->ops->probe(h->ddf[h->cur], make_params(h), h->has_force, (const long long *)d, count, df, df + count, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rho, df, (size_t)count * 4, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(u, df + count, (size_t)count * 12, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    cudaFree(d);
+    LBM_CUDA_TRY(e);
+    LBM_CUDA_TRY(e2);
+    return LBM_OK;
+}
+
 int lbm_read_ddf(lbm_t *h, int i, void *out) {
     if (int rc = enter(h)) return rc;
     if (!h->inited) return fail(LBM_E_STATE, "lbm_read_ddf: call lbm_init first");

@@ -18,6 +18,8 @@ struct UnitOps {
     cudaError_t (*read)(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st);
     const char *(*name)(int V, int coll, bool force);
     int (*bulk_tile_cells)();     // cells per tile of the staged kernel
+    cudaError_t (*probe)(const void *A, const Params &p, bool force, const long long *cells, int count, float *rho, float *u,
+                         cudaStream_t st);
 };
 
 const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)

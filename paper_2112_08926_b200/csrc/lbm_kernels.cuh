@@ -282,4 +282,32 @@ read_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, flo
     }
 }
 
+// ---- read-out at selected cells (R12), for probes in long runs ---------------------------------------
+template <int Q, int F, bool FORCE>
+__global__ void __launch_bounds__(128)
+probe_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, const long long *__restrict__ cells, int count,
+                   float *__restrict__ rho_out, float *__restrict__ u_out) {
+    typedef Elem<F> E;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    const long long n = cells[k], N = p.N;
+    float rho, j[3], u[3];
+    if (__ldg(p.flags + n) & FLAG_FIXED) {
+        rho = __ldg(p.rho0 + n);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) u[a] = __ldg(p.u0 + a * N + n);
+    } else {
+        float f[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) f[i] = E::ld1(A + (long long)i * N + n);
+        moments<Q>(f, rho, j);
+        const float Fv[3] = {p.fx, p.fy, p.fz};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) u[a] = __fdiv_rn(FORCE ? fma_(-0.5f, Fv[a], j[a]) : j[a], rho);
+    }
+    rho_out[k] = rho;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) u_out[a * count + k] = u[a];
+}
+
 }  // namespace lbmk

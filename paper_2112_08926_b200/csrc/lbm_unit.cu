@@ -118,6 +118,14 @@ cudaError_t read(const void *A, const Params &p, bool force, float *rho, float *
     return cudaGetLastError();
 }
 
+cudaError_t probe(const void *A, const Params &p, bool force, const long long *cells, int count, float *rho, float *u, cudaStream_t st) {
+    const int blocks = (count + 127) / 128;
+    if (force) probe_rho_u_kernel<Q, F, true><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
+    else probe_rho_u_kernel<Q, F, false><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
+    count_launch();
+    return cudaGetLastError();
+}
+
 const char *name(int V, int coll, bool force) {
     (void)coll;
     static const char *names[4][2] = {
@@ -137,6 +145,6 @@ int bulk_tile_cells() { return 2 * BULK_NT; }
 }  // namespace
 
 extern const UnitOps LBM_UNIT_SYMBOL;
-const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells};
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells, probe};
 
 }  // namespace lbmk

@@ -73,3 +73,21 @@ def test_sizes():
     assert lbm.bytes_per_cell(19, "FP32") == 153 and lbm.bytes_per_cell(19, "FP16S") == 77
     assert lbm.bytes_per_cell(27, "FP32") == 217 and lbm.bytes_per_cell(9, "P16_2C") == 37
     assert lbm.ddf_buffer_bytes(32, 32, 32, 19, "FP16C") == 32 ** 3 * 19 * 2
+
+
+def test_read_rho_u_at_equals_full_readout():
+    import workloads as wl
+    w = wl.perturbed_equilibrium(32, 6, 5, seed=9)
+    w = wl.random_walls(w, 0.1, seed=2, moving_fraction=0.5)
+    w.force = (1e-5, 0.0, 2e-5)
+    for name in ("FP32", "FP16C"):
+        s = lbm.from_workload(w, name)
+        s.step(7)
+        rho, u = s.read_rho_u()
+        cells = np.array([0, 5, 31, 32, 500, w.n_cells - 1, 77], np.int64)
+        r, v = s.read_rho_u_at(cells)
+        assert np.array_equal(r.view(np.uint32), rho[cells].view(np.uint32))
+        assert np.array_equal(v.view(np.uint32), u[:, cells].view(np.uint32))
+        with pytest.raises(lbm.LbmError):
+            s.read_rho_u_at([w.n_cells])
+        s.close()
