@@ -31,6 +31,7 @@ struct lbm {
     bool owns_ddf, bound;
     int cur;                   // index of the buffer holding the current state
     float *rho0, *u0;          // device copies of the init fields, kept only when the box has walls
+    unsigned *bounce;          // device, N words: which directions bounce (lbm_lattice.cuh), only when the box has walls
     long long steps;
     bool inited;
     int V;                     // stream_collide variant in use: 1, 2, 4 cells per thread or LBM_VARIANT_BULK
@@ -73,6 +74,7 @@ Params make_params(const lbm *h) {
     p.flags = h->flags;
     p.rho0 = h->rho0;
     p.u0 = h->u0;
+    p.bounce = h->bounce;
     return p;
 }
 
@@ -230,9 +232,10 @@ int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
         return LBM_OK;
     }
     unsigned char *tmp = nullptr;
+    if (!h->bounce) LBM_CUDA_TRY(cudaMalloc((void **)&h->bounce, (size_t)h->N * 4));
     LBM_CUDA_TRY(cudaMalloc((void **)&tmp, (size_t)h->N));
     cudaError_t e = cudaMemcpyAsync(tmp, flags, (size_t)h->N, cudaMemcpyHostToDevice, h->stream);
-    if (e == cudaSuccess) e = lbmk::launch_mark_near(h->q, tmp, h->flags, h->nx, h->ny, h->nz, h->stream);
+    if (e == cudaSuccess) e = lbmk::launch_mark_near(h->q, tmp, h->flags, h->bounce, h->nx, h->ny, h->nz, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     cudaFree(tmp);
     LBM_CUDA_TRY(e);
@@ -249,6 +252,7 @@ static int init_from_device(lbm *h, const float *rho_dev, const float *u_dev) {
         if (h->u0 != u_dev) LBM_CUDA_TRY(cudaMemcpyAsync(h->u0, u_dev, (size_t)h->N * 12, cudaMemcpyDeviceToDevice, h->stream));
         r = h->rho0;
         u = h->u0;
+        LBM_CUDA_TRY(lbmk::launch_mark_moving(h->q, h->bounce, h->u0, h->nx, h->ny, h->nz, h->stream));
     }
     LBM_CUDA_TRY(h->ops->init(h->ddf[0], h->ddf[1], r, u, h->N, h->stream));
     h->cur = 0;
@@ -381,6 +385,7 @@ int lbm_destroy(lbm_t *h) {
     if (h->flags) cudaFree(h->flags);
     if (h->rho0) cudaFree(h->rho0);
     if (h->u0) cudaFree(h->u0);
+    if (h->bounce) cudaFree(h->bounce);
     (void)cudaGetLastError();
     delete h;
     return LBM_OK;

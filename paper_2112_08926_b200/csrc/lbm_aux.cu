@@ -17,13 +17,14 @@ long long launches() { return g_launches.load(); }
 // the paper's kernel gathers.
 template <int Q>
 __global__ void __launch_bounds__(256) mark_near_kernel(const unsigned char *__restrict__ in, unsigned char *__restrict__ out,
-                                                        int nx, int ny, int nz) {
+                                                        unsigned *__restrict__ bounce, int nx, int ny, int nz) {
     typedef Lat<Q> L;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y, z = blockIdx.z;
     if (x >= nx) return;
     const long long n = x + (long long)nx * (y + (long long)ny * z);
     unsigned fl = in[n] & FLAG_FIXED;
+    unsigned mask = 0;                                       // bit i: the pull source of direction i is a wall cell
     if (!fl) {
         unsigned near = 0;
 #pragma unroll
@@ -32,18 +33,58 @@ __global__ void __launch_bounds__(256) mark_near_kernel(const unsigned char *__r
             xs = xs < 0 ? nx - 1 : xs >= nx ? 0 : xs;
             ys = ys < 0 ? ny - 1 : ys >= ny ? 0 : ys;
             zs = zs < 0 ? nz - 1 : zs >= nz ? 0 : zs;
-            near |= in[xs + (long long)nx * (ys + (long long)ny * zs)] & FLAG_WALL;
+            const unsigned wsrc = in[xs + (long long)nx * (ys + (long long)ny * zs)] & FLAG_WALL;
+            near |= wsrc;
+            mask |= wsrc << i;
         }
         if (near) fl |= FLAG_NEAR;
     }
     out[n] = (unsigned char)fl;
+    bounce[n] = mask;
 }
 
-cudaError_t launch_mark_near(int q, const unsigned char *in, unsigned char *out, int nx, int ny, int nz, cudaStream_t st) {
+cudaError_t launch_mark_near(int q, const unsigned char *in, unsigned char *out, unsigned *bounce, int nx, int ny, int nz,
+                             cudaStream_t st) {
     const dim3 block(256), grid((nx + 255) / 256, ny, nz);
-    if (q == 9) mark_near_kernel<9><<<grid, block, 0, st>>>(in, out, nx, ny, nz);
-    else if (q == 19) mark_near_kernel<19><<<grid, block, 0, st>>>(in, out, nx, ny, nz);
-    else if (q == 27) mark_near_kernel<27><<<grid, block, 0, st>>>(in, out, nx, ny, nz);
+    if (q == 9) mark_near_kernel<9><<<grid, block, 0, st>>>(in, out, bounce, nx, ny, nz);
+    else if (q == 19) mark_near_kernel<19><<<grid, block, 0, st>>>(in, out, bounce, nx, ny, nz);
+    else if (q == 27) mark_near_kernel<27><<<grid, block, 0, st>>>(in, out, bounce, nx, ny, nz);
+    else return cudaErrorInvalidValue;
+    count_launch();
+    return cudaGetLastError();
+}
+
+// bounce[n] bit 31 := one of the wall cells this cell bounces on has a non-zero velocity (R9); run by lbm_init,
+// when the wall velocities are known.  Cells whose walls all rest never load a wall velocity in the time step.
+template <int Q>
+__global__ void __launch_bounds__(256) mark_moving_kernel(unsigned *__restrict__ bounce, const float *__restrict__ u0, int nx, int ny,
+                                                          int nz) {
+    typedef Lat<Q> L;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, z = blockIdx.z;
+    if (x >= nx) return;
+    const long long N = (long long)nx * ny * nz, n = x + (long long)nx * (y + (long long)ny * z);
+    unsigned m = bounce[n] & 0x7FFFFFFFu;
+    if (m == 0) return;
+    bool moving = false;
+#pragma unroll
+    for (int i = 1; i < Q; ++i) {
+        if (!((m >> i) & 1u)) continue;
+        int xs = x - L::c(i, 0), ys = y - L::c(i, 1), zs = z - L::c(i, 2);
+        xs = xs < 0 ? nx - 1 : xs >= nx ? 0 : xs;
+        ys = ys < 0 ? ny - 1 : ys >= ny ? 0 : ys;
+        zs = zs < 0 ? nz - 1 : zs >= nz ? 0 : zs;
+        const long long src = xs + (long long)nx * (ys + (long long)ny * zs);
+        moving |= u0[src] != 0.0f || u0[N + src] != 0.0f || u0[2 * N + src] != 0.0f;
+    }
+    bounce[n] = m | (moving ? 0x80000000u : 0u);
+}
+
+cudaError_t launch_mark_moving(int q, unsigned *bounce, const float *u0, int nx, int ny, int nz, cudaStream_t st) {
+    const dim3 block(256), grid((nx + 255) / 256, ny, nz);
+    if (q == 9) mark_moving_kernel<9><<<grid, block, 0, st>>>(bounce, u0, nx, ny, nz);
+    else if (q == 19) mark_moving_kernel<19><<<grid, block, 0, st>>>(bounce, u0, nx, ny, nz);
+    else if (q == 27) mark_moving_kernel<27><<<grid, block, 0, st>>>(bounce, u0, nx, ny, nz);
     else return cudaErrorInvalidValue;
     count_launch();
     return cudaGetLastError();

@@ -25,8 +25,9 @@
 //     halo copy per shifted direction fills the pad in front of / behind the segment;
 //   * results are encoded in registers and stored directly (one aligned 32/64-bit store per direction and cell
 //     pair, 128/256 contiguous bytes per warp): stores need no latency hiding, so they need no staging;
-//   * cells with any flag bit set (wall, or next to a wall; lbm_set_flags marks the latter) take the per-cell
-//     path of lbm_kernels.cuh (PullDirWall: neighbour-flag gathers, bounce-back, moving wall).
+//   * cell pairs with any flag bit set (wall, equilibrium boundary, or next to a wall; lbm_set_flags marks the latter)
+//     are pulled from the stage like the others and then fixed up cell by cell: fixed cells are not written, a cell
+//     next to a wall replaces its bounced links from a precomputed per-cell word (bounce_links below).
 // Arithmetic, operation order and codecs are those of lbm_lattice.cuh / lbm_codecs.cuh: the stored results
 // are bit-identical to stream_collide_kernel's and to the oracle's.
 #pragma once
@@ -250,6 +251,44 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     }
 }
 
+// Halfway bounce-back for one cell next to a wall (R3; moving wall R9).  f holds the q
+// directions pulled as if every source were fluid; the links whose source is a wall cell -- one precomputed word per
+// cell, written by lbm_set_flags -- are replaced by the cell's own opposite population, all loads independent of
+// one another.  Wall velocities are loaded only for cells one of whose walls moves (bit 31, set by lbm_init).
+template <int Q, int F>
+__device__ __forceinline__ void bounce_links(const typename Elem<F>::T *__restrict__ A, const Params &p, long long n, int x, int y,
+                                             int z, float (&f)[Q]) {
+    typedef Lat<Q> L;
+    typedef Elem<F> E;
+    const unsigned m = __ldg(p.bounce + n);
+#pragma unroll
+    for (int i = 1; i < Q; ++i)
+        if ((m >> i) & 1u) f[i] = E::ld1(A + (long long)L::opp(i) * p.N + n);
+    if (!(m >> 31)) return;
+#pragma unroll
+    for (int i = 1; i < Q; ++i) {                                               // static indices: f stays in registers
+        if (!((m >> i) & 1u)) continue;
+        int xs = x - L::c(i, 0), ys = y - L::c(i, 1), zs = z - L::c(i, 2);
+        xs = xs < 0 ? p.nx - 1 : xs >= p.nx ? 0 : xs;
+        ys = ys < 0 ? p.ny - 1 : ys >= p.ny ? 0 : ys;
+        zs = zs < 0 ? p.nz - 1 : zs >= p.nz ? 0 : zs;
+        const long long src = xs + (long long)p.nx * (ys + (long long)p.ny * zs);
+        const float v[3] = {__ldg(p.u0 + src), __ldg(p.u0 + p.N + src), __ldg(p.u0 + 2 * p.N + src)};
+        if (v[0] != 0.0f || v[1] != 0.0f || v[2] != 0.0f) {                     // rho_w = 1; a resting wall adds nothing
+            float sdot = 0.0f;                                                  // c_i . u_w as cdot<Q, i> of lbm_lattice.cuh
+            bool first = true;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                if (L::c(i, a) == 0) continue;
+                const float term = L::c(i, a) > 0 ? v[a] : -v[a];
+                sdot = first ? term : add(sdot, term);
+                first = false;
+            }
+            f[i] = add(f[i], mul(L::w6(i), sdot));
+        }
+    }
+}
+
 template <int Q, int F, int NT, bool FORCE>
 __global__ void __launch_bounds__(NT, 2)
 stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p,
@@ -321,7 +360,8 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             if (fast) PullStaged<Q, F, NT, PC, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
             // codes outside the fast decoders' domain (posits: a regime of ones): this pair goes through Codec<F>
             const bool exact = PC::CHECK != 0 && ((acc | (acc >> 16)) & PC::CHECK) != 0;
-            if (exact) {
+            const bool slow = active && fl != 0;            // a fixed cell or a wall among the pull sources (below)
+            if (exact || slow) {
                 unsigned dummy = 0;
                 PullStaged<Q, F, NT, PairCodec<-1 - F>, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, dummy);
             }
@@ -346,28 +386,18 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
                     for (int i = 0; i < Q; ++i)
                         *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = Codec<F>::enc(f[0][i]) | (Codec<F>::enc(f[1][i]) << 16);
                 }
-            } else {
-                if (active) {
-                    // a wall cell or a wall among the pull sources: cell by cell from global memory (lbm_kernels.cuh)
-                    const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
-                    const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
-                    const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
-                    long long rows[3][3];
+            } else if (slow) {
+                // f holds every direction pulled from the stage as if there were no wall.  Cell by cell: fixed cells are
+                // not written (R15); a cell next to a wall replaces its bounced links (R3, R9).
 #pragma unroll
-                    for (int a = 0; a < 3; ++a)
+                for (int j = 0; j < 2; ++j) {
+                    const unsigned cf = (fl >> (8 * j)) & 0xFFu;
+                    if (cf & FLAG_FIXED) continue;
+                    const long long n = own + j;
+                    if (cf & FLAG_NEAR) bounce_links<Q, F>(A, p, n, c.x0 + xl + j, y, z, f[j]);
+                    collide_bgk<Q, FORCE, 0>(f[j], p);
 #pragma unroll
-                        for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
-#pragma unroll 1
-                    for (int j = 0; j < 2; ++j) {
-                        if ((fl >> (8 * j)) & FLAG_FIXED) continue;             // wall (and E) cells are not updated
-                        const int x = c.x0 + xl + j;
-                        const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
-                        float gq[Q];
-                        PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, gq);
-                        collide_bgk<Q, FORCE, 0>(gq, p);
-#pragma unroll
-                        for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + own + j, gq[i]);
-                    }
+                    for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + n, f[j][i]);
                 }
             }
         }

@@ -25,7 +25,9 @@ struct UnitOps {
 const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)
 
 // lbm_aux.cu
-cudaError_t launch_mark_near(int q, const unsigned char *in, unsigned char *out, int nx, int ny, int nz, cudaStream_t st);
+cudaError_t launch_mark_near(int q, const unsigned char *in, unsigned char *out, unsigned *bounce, int nx, int ny, int nz,
+                             cudaStream_t st);
+cudaError_t launch_mark_moving(int q, unsigned *bounce, const float *u0, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t launch_codec(int fmt, bool encode, const void *in, void *out, long long count, cudaStream_t st);
 struct EncEntry;
 cudaError_t enc_table(int fmt, const EncEntry **out, cudaStream_t st);   // device pointer to the format's encoder table (built on first use)
