@@ -219,6 +219,15 @@ __global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *
 #endif
         if (v < 65536) {
             unsigned c = (unsigned)v, c2 = (c * 40503u + 7u) & 0xFFFFu;
+            if constexpr (PC::CHECK != 0) {                                     // the full-range decoders: every code
+                typedef typename PC::Full FD;
+                const float r = __fmul_rn(Codec<F>::dec(c), up), r2 = __fmul_rn(Codec<F>::dec(c2), up);
+                float a, d;
+                FD::dec2(c | (c2 << 16), a, d);
+                const float e = FD::dec1((int)(short)c);
+                bad += (__float_as_uint(a) != __float_as_uint(r)) + (__float_as_uint(d) != __float_as_uint(r2)) +
+                       (__float_as_uint(e) != __float_as_uint(r));
+            }
             if (PC::CHECK) { c2 &= ~PC::CHECK; if (c & PC::CHECK) continue; }  // outside the fast decoders' domain: the kernel falls back
             const float r = __fmul_rn(Codec<F>::dec(c), up), r2 = __fmul_rn(Codec<F>::dec(c2), up);
             float a, d;

@@ -125,6 +125,12 @@ struct BulkShape {
     static_assert(STAGEB % 16 == 0 && ROWB % 16 == 0, "bulk copies need 16-byte alignment");
 };
 
+// decode policy of the full-range posit decoders: PairCodec<F>::Full, recording the codes it sees like PairCodec<F>
+template <int F>
+struct FullRange : PairCodec<F>::Full {
+    static constexpr unsigned CHECK = PairCodec<F>::CHECK;
+};
+
 // shared-memory access (addresses are "thread base + immediate")
 __device__ __forceinline__ unsigned lds_u32(const char *p) { return *reinterpret_cast<const unsigned *>(p); }
 __device__ __forceinline__ int lds_s16(const char *p) { return (int)*reinterpret_cast<const short *>(p); }
@@ -251,11 +257,17 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     }
 }
 
+// x 2^SC, exact (the staged kernel keeps FP16S / P16_0S values scaled, collide_bgk<.., SC>)
+template <int SC>
+__device__ __forceinline__ float scaled(float v) { return SC == 0 ? v : mul(v, pow2f(SC)); }
+
 // Halfway bounce-back for one cell next to a wall (R3; moving wall R9).  f holds the q
 // directions pulled as if every source were fluid; the links whose source is a wall cell -- one precomputed word per
 // cell, written by lbm_set_flags -- are replaced by the cell's own opposite population, all loads independent of
 // one another.  Wall velocities are loaded only for cells one of whose walls moves (bit 31, set by lbm_init).
-template <int Q, int F>
+// f is in the kernel's 2^SC scaling; the bounced values and the moving-wall term (evaluated as R9 states) are
+// scaled exactly.
+template <int Q, int F, int SC>
 __device__ __forceinline__ void bounce_links(const typename Elem<F>::T *__restrict__ A, const Params &p, long long n, int x, int y,
                                              int z, float (&f)[Q]) {
     typedef Lat<Q> L;
@@ -263,7 +275,7 @@ __device__ __forceinline__ void bounce_links(const typename Elem<F>::T *__restri
     const unsigned m = __ldg(p.bounce + n);
 #pragma unroll
     for (int i = 1; i < Q; ++i)
-        if ((m >> i) & 1u) f[i] = E::ld1(A + (long long)L::opp(i) * p.N + n);
+        if ((m >> i) & 1u) f[i] = scaled<SC>(E::ld1(A + (long long)L::opp(i) * p.N + n));
     if (!(m >> 31)) return;
 #pragma unroll
     for (int i = 1; i < Q; ++i) {                                               // static indices: f stays in registers
@@ -284,7 +296,7 @@ __device__ __forceinline__ void bounce_links(const typename Elem<F>::T *__restri
                 sdot = first ? term : add(sdot, term);
                 first = false;
             }
-            f[i] = add(f[i], mul(L::w6(i), sdot));
+            f[i] = add(f[i], scaled<SC>(mul(L::w6(i), sdot)));
         }
     }
 }
@@ -330,6 +342,7 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
         if (t < g.n_tiles) issue_tile_loads<Q, F, NT>(A, p, g, (int)t, smem_base + s * SH::STAGEB, bar_full + s * 8, warp, lane);
     }
 
+    bool full_mode = false;                              // posits: this thread currently needs the full-range decoders
     int k = 0;
     for (int t = blockIdx.x; t < g.n_tiles; t += stride, ++k) {
         const int s = k % S;
@@ -357,34 +370,36 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             float f[2][Q];
             unsigned acc = 0;
             const char *base = stage + SH::PAD + r * pitch;
-            if (fast) PullStaged<Q, F, NT, PC, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
-            // codes outside the fast decoders' domain (posits: a regime of ones): this pair goes through Codec<F>
-            const bool exact = PC::CHECK != 0 && ((acc | (acc >> 16)) & PC::CHECK) != 0;
-            const bool slow = active && fl != 0;            // a fixed cell or a wall among the pull sources (below)
-            if (exact || slow) {
-                unsigned dummy = 0;
-                PullStaged<Q, F, NT, PairCodec<-1 - F>, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, dummy);
+            bool warp_full = false;
+            if constexpr (PC::CHECK != 0) warp_full = __any_sync(0xffffffffu, full_mode);   // one decoder per warp where possible
+            if (active) {                                   // every direction from the stage, as if no wall were near
+                if constexpr (PC::CHECK != 0) {
+                    // posits: the cheap decoders cover a regime of zeros (|f| < 2^-7).  A thread that met other codes
+                    // makes its warp pull with the full-range decoders until its pairs are free of such codes again
+                    // (flows are smooth: the choice rarely changes from one pair to the next)
+                    if (!warp_full) PullStaged<Q, F, NT, PC, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
+                    if (warp_full || ((acc | (acc >> 16)) & PC::CHECK) != 0) {
+                        acc = 0;
+                        PullStaged<Q, F, NT, FullRange<F>, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
+                    }
+                    full_mode = ((acc | (acc >> 16)) & PC::CHECK) != 0;
+                } else {
+                    PullStaged<Q, F, NT, PC, 0>::run(base + xl * ES, base + el * ES, base + er * ES, f, acc);
+                }
             }
+            const bool slow = active && fl != 0;            // a fixed cell or a wall among the pull sources (below)
             if ((it + 1) * NT >= pairs) {                                       // last trip: the warp has its values in registers,
                 __syncwarp();                                                   // the stage may be refilled
                 if (lane == 0) mbar_arrive(bar_empty + s * 8);
             }
             if (fast) {
                 T *o = B + own;
-                if (!exact) {
-                    collide_bgk<Q, FORCE, SC>(f[0], p);
-                    collide_bgk<Q, FORCE, SC>(f[1], p);
+                collide_bgk<Q, FORCE, SC>(f[0], p);
+                collide_bgk<Q, FORCE, SC>(f[1], p);
 #pragma unroll
-                    for (int i = 0; i < Q; ++i) {
-                        if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
-                        else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PC::enc2(f[0][i], f[1][i], tab);
-                    }
-                } else if constexpr (ES == 2) {
-                    collide_bgk<Q, FORCE, 0>(f[0], p);
-                    collide_bgk<Q, FORCE, 0>(f[1], p);
-#pragma unroll
-                    for (int i = 0; i < Q; ++i)
-                        *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = Codec<F>::enc(f[0][i]) | (Codec<F>::enc(f[1][i]) << 16);
+                for (int i = 0; i < Q; ++i) {
+                    if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
+                    else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PC::enc2(f[0][i], f[1][i], tab);
                 }
             } else if (slow) {
                 // f holds every direction pulled from the stage as if there were no wall.  Cell by cell: fixed cells are
@@ -394,10 +409,13 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
                     const unsigned cf = (fl >> (8 * j)) & 0xFFu;
                     if (cf & FLAG_FIXED) continue;
                     const long long n = own + j;
-                    if (cf & FLAG_NEAR) bounce_links<Q, F>(A, p, n, c.x0 + xl + j, y, z, f[j]);
-                    collide_bgk<Q, FORCE, 0>(f[j], p);
+                    if (cf & FLAG_NEAR) bounce_links<Q, F, SC>(A, p, n, c.x0 + xl + j, y, z, f[j]);
+                    collide_bgk<Q, FORCE, SC>(f[j], p);
 #pragma unroll
-                    for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + n, f[j][i]);
+                    for (int i = 0; i < Q; ++i) {
+                        if constexpr (ES == 4) B[(long long)i * p.N + n] = f[j][i];
+                        else B[(long long)i * p.N + n] = (T)PC::enc1(f[j][i], tab);
+                    }
                 }
             }
         }

@@ -159,7 +159,7 @@ struct Codec<F_P16_2C> {
 //   dec2(w)   both codes of a word;  enc2(a, b) packs the codes of a (low) and b (high).
 //   TABLE     enc2 reads the format's 512-entry encoder table (EncEntry, below) from shared memory;
 //   CHECK     codes with (code & CHECK) != 0 are outside the domain of dec1 / dec2: the caller ORs the raw words
-//             together and, if a CHECK bit shows up, redoes the cell with Codec<F> (rare by construction).
+//             together and, if a CHECK bit shows up, decodes again with PairCodec<F>::Full (all codes, dearer).
 // Every function returns bit for bit what Codec<F>::dec / enc return (times 2^SC).
 struct EncEntry {
     unsigned add, mult, base, tmax;     // code = base + hi32(min(bits(X) + add, tmax) * mult)
@@ -178,6 +178,7 @@ struct PairCodec {
     static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *) {
         return Codec<F>::enc(a) | (Codec<F>::enc(b) << 16);
     }
+    static __device__ __forceinline__ unsigned enc1(float a, const EncEntry *) { return Codec<F>::enc(a); }   // one code
 };
 
 template <int SCALE>
@@ -195,6 +196,7 @@ struct PairHalf {
         const __half2 h = __floats2half2_rn(a, b);          // one F2FP.F16.F32.PACK_AB, round-to-nearest-even
         return *reinterpret_cast<const unsigned *>(&h);
     }
+    static __device__ __forceinline__ unsigned enc1(float a, const EncEntry *) { return __half_as_ushort(__float2half_rn(a)); }
 };
 template <>
 struct PairCodec<F_FP16> : PairHalf<0> {};
@@ -228,6 +230,7 @@ struct PairCodec<F_FP16C> {
         const unsigned signs = __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x7632);
         return (mags & 0x7FFF7FFFu) | (signs & 0x80008000u);
     }
+    static __device__ __forceinline__ unsigned enc1(float a, const EncEntry *t) { return enc2(a, a, t) & 0xFFFFu; }
 };
 
 // ---- posits on pairs ------------------------------------------------------------------------------------
@@ -258,11 +261,34 @@ __device__ __forceinline__ unsigned enc_by_table(float X, const EncEntry *tab) {
 //   es = 1   word = 2 b - 0x43000000        (exponent field 120 - 2k + e, scale 2^-7 included);
 //   es = 2   word = 4 b + 0x40000000        (exponent field 124 - 4r + e; mod 2^32);
 // max(b, .) maps the zero code to zero.  A regime of ONES (bit 14 set, |f| >= 2^-7) is not handled here: CHECK.
+// Full-range posit decoders (both regime signs), used where the zero-regime decoders above do not apply.
+// Sign-extending the 15 magnitude bits from bit 14 gives t = n for a regime of zeros and t = -(2^15 - n) for a regime
+// of ones; |t| normalised (int -> float) has the regime length in its exponent and, for ones, the COMPLEMENT of the
+// payload [e F] in its mantissa: 2^15 - n = 2^(L+1) - P for a payload P of L bits, so its float is 2^L (2 - P/2^L) and
+// subtracting the word from a constant both negates the exponent and turns 1 - P/2^L back into P/2^L.  Hence
+//   regime of zeros: word = MUL * b - KZ,      regime of ones: word = KO - MUL * b     (mod 2^32, b = float word of t)
+// with MUL = 2^es moving the exponent bit(s) from the mantissa top into the exponent field.
+template <int MUL, unsigned KZ, unsigned KO, unsigned FLOOR>
+struct PositFull {
+    static __device__ __forceinline__ float word(int t, unsigned sign) {        // t = magnitude sign-extended from bit 14
+        const unsigned b = __float_as_uint(__int2float_rn(t));
+        const unsigned wz = max(b, FLOOR) * (unsigned)MUL - KZ;                 // FLOOR: the zero code gives zero
+        const unsigned wo = KO - b * (unsigned)MUL;
+        return __uint_as_float(((t < 0 ? wo : wz) & 0x7FFFFFFFu) | (sign & 0x80000000u));
+    }
+    static __device__ __forceinline__ float dec1(int c) { return word((c << 17) >> 17, (unsigned)c << 16); }
+    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
+        a = word((int)(w << 17) >> 17, w << 16);
+        b = word((int)(w << 1) >> 17, w);
+    }
+};
+
 template <>
 struct PairCodec<F_P16_0S> {
     static constexpr int SC = -1;           // decoded = n 2^-22 = f / 2: one multiply, the factor 2 rides on SC
     static constexpr bool TABLE = true;
     static constexpr unsigned CHECK = 0x4000u;
+    typedef PositFull<1, 0x0B000000u, 0x02000000u, 0x0B000000u> Full;           // same scaling: f / 2
     static __device__ __forceinline__ float sm2f(unsigned t) {      // t = sign-extended code
         return __fmul_rn(__uint_as_float(t & 0x80007FFFu), __uint_as_float(0x7F000000u));   // * 2^127, exact
     }
@@ -274,6 +300,7 @@ struct PairCodec<F_P16_0S> {
     static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *tab) {
         return __byte_perm(enc_by_table<false>(a, tab), enc_by_table<false>(b, tab), 0x5410);
     }
+    static __device__ __forceinline__ unsigned enc1(float a, const EncEntry *tab) { return enc_by_table<false>(a, tab) & 0xFFFFu; }
 };
 
 template <int MUL, unsigned OFF, unsigned FLOOR, unsigned CHK>
@@ -295,30 +322,13 @@ struct PairPositLow {
     static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *tab) {
         return __byte_perm(enc_by_table<CHK == 0>(a, tab), enc_by_table<CHK == 0>(b, tab), 0x5410);
     }
+    static __device__ __forceinline__ unsigned enc1(float a, const EncEntry *tab) { return enc_by_table<CHK == 0>(a, tab) & 0xFFFFu; }
 };
 template <>
-struct PairCodec<F_P16_1S> : PairPositLow<2, 0xBD000000u /* -0x43000000 */, 0x21800000u, 0x4000u> {};
+struct PairCodec<F_P16_1S> : PairPositLow<2, 0xBD000000u /* -0x43000000 */, 0x21800000u, 0x4000u> {
+    typedef PositFull<2, 0x51000000u, 0xC9000000u, 0x28800000u> Full;
+};
 template <>
 struct PairCodec<F_P16_2C> : PairPositLow<4, 0x40000000u, 0x30000000u, 0u> {};
-
-// PairCodec<-1 - F>: the exact fall-back decoders (Codec<F> on every code), used when a CHECK bit shows up
-template <int F>
-struct ExactPair {
-    static constexpr int SC = 0;
-    static constexpr bool TABLE = false;
-    static constexpr unsigned CHECK = 0;
-    static __device__ __forceinline__ float dec1(int c) { return Codec<F>::dec((unsigned)c & 0xFFFFu); }
-    static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
-        a = Codec<F>::dec(w & 0xFFFFu);
-        b = Codec<F>::dec(w >> 16);
-    }
-};
-template <> struct PairCodec<-1 - F_FP16S> : ExactPair<F_FP16S> {};
-template <> struct PairCodec<-1 - F_FP16C> : ExactPair<F_FP16C> {};
-template <> struct PairCodec<-1 - F_P16_0S> : ExactPair<F_P16_0S> {};
-template <> struct PairCodec<-1 - F_P16_1S> : ExactPair<F_P16_1S> {};
-template <> struct PairCodec<-1 - F_P16_2C> : ExactPair<F_P16_2C> {};
-template <> struct PairCodec<-1 - F_FP16> : ExactPair<F_FP16> {};
-template <> struct PairCodec<-1 - F_FP32> : ExactPair<F_FP16> {};       // never used (FP32 has no codes); keeps templates well-formed
 
 }  // namespace lbmk
