@@ -101,7 +101,7 @@ int ensure_ddf(lbm *h) {
 }
 
 // Kernel variant.  Automatic choice, from the bandwidth sweep recorded in DESIGN.md section 6:
-//   * FP32 storage: the per-thread kernel (it runs at the HBM roofline);
+//   * FP32 storage, no flagged cells: the per-thread kernel (it runs at the HBM roofline);
 //   * 16-bit formats, D3Q19 / D3Q27, rows 16-cell aligned and >= 64 cells, box >= 2^20 cells: the
 //     shared-memory-staged kernel (lbm_bulk.cuh), which lifts them out of the issue bound;
 //   * D2Q9 (9 streams: the staged kernel's per-tile bookkeeping does not pay) and small boxes (L2-resident,
@@ -114,7 +114,9 @@ int pick_variant(const lbm *h) {
     }
     const bool bulk_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->bulk_tile_cells() - 1) / h->ops->bulk_tile_cells()) * h->ny * h->nz <= 0x7FFFFFFFLL;
     if (want == LBM_VARIANT_BULK && bulk_ok) return LBM_VARIANT_BULK;
-    if (want == 0 && bulk_ok && h->fmt != LBM_FP32 && h->q != LBM_D2Q9 && h->nx >= 64 && h->N >= (1LL << 20)) return LBM_VARIANT_BULK;
+    // (FP32 storage in a box with flagged cells also gains: the staged kernel's near-wall path has no serial gathers)
+    if (want == 0 && bulk_ok && (h->fmt != LBM_FP32 || h->has_walls) && h->q != LBM_D2Q9 && h->nx >= 64 && h->N >= (1LL << 20))
+        return LBM_VARIANT_BULK;
     if (want != 1 && want != 2 && want != 4) want = (h->q == LBM_D2Q9 && h->fmt != LBM_FP32) ? 4 : 2;
     while (want > 1 && h->nx % want != 0) want >>= 1;
     return want;
