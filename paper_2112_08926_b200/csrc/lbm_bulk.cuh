@@ -269,10 +269,9 @@ __device__ __forceinline__ float scaled(float v) { return SC == 0 ? v : mul(v, p
 // scaled exactly.
 template <int Q, int F, int SC>
 __device__ __forceinline__ void bounce_links(const typename Elem<F>::T *__restrict__ A, const Params &p, long long n, int x, int y,
-                                             int z, float (&f)[Q]) {
+                                             int z, unsigned m, float (&f)[Q]) {
     typedef Lat<Q> L;
     typedef Elem<F> E;
-    const unsigned m = __ldg(p.bounce + n);
 #pragma unroll
     for (int i = 1; i < Q; ++i)
         if ((m >> i) & 1u) f[i] = scaled<SC>(E::ld1(A + (long long)L::opp(i) * p.N + n));
@@ -367,6 +366,10 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             unsigned fl = 0;
             if (active) fl = *reinterpret_cast<const unsigned short *>(stage + Q * SH::ROWB + r * w + xl);
             const bool fast = active && fl == 0;
+            // near-wall cells: which links bounce (one word per cell, lbm_set_flags); loaded now, needed after the pull
+            unsigned bm[2] = {0u, 0u};
+            if (fl & FLAG_NEAR) bm[0] = __ldg(p.bounce + own);
+            if (fl & (FLAG_NEAR << 8)) bm[1] = __ldg(p.bounce + own + 1);
             float f[2][Q];
             unsigned acc = 0;
             const char *base = stage + SH::PAD + r * pitch;
@@ -405,11 +408,12 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
                 // f holds every direction pulled from the stage as if there were no wall.  Cell by cell: fixed cells are
                 // not written (R15); a cell next to a wall replaces its bounced links (R3, R9).
 #pragma unroll
+                for (int j = 0; j < 2; ++j)                                     // all bounced loads of both cells first
+                    if (bm[j]) bounce_links<Q, F, SC>(A, p, own + j, c.x0 + xl + j, y, z, bm[j], f[j]);
+#pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    const unsigned cf = (fl >> (8 * j)) & 0xFFu;
-                    if (cf & FLAG_FIXED) continue;
+                    if ((fl >> (8 * j)) & FLAG_FIXED) continue;
                     const long long n = own + j;
-                    if (cf & FLAG_NEAR) bounce_links<Q, F, SC>(A, p, n, c.x0 + xl + j, y, z, f[j]);
                     collide_bgk<Q, FORCE, SC>(f[j], p);
 #pragma unroll
                     for (int i = 0; i < Q; ++i) {
