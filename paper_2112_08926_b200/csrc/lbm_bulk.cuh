@@ -395,30 +395,34 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
                 __syncwarp();                                                   // the stage may be refilled
                 if (lane == 0) mbar_arrive(bar_empty + s * 8);
             }
-            if (fast) {
-                T *o = B + own;
+            if (slow) {
+                // f holds every direction pulled from the stage as if there were no wall: a cell next to a wall replaces
+                // its bounced links (R3, R9), all loads of both cells in flight together
+#pragma unroll
+                for (int j = 0; j < 2; ++j)
+                    if (bm[j]) bounce_links<Q, F, SC>(A, p, own + j, c.x0 + xl + j, y, z, bm[j], f[j]);
+            }
+            if (active) {
+                // one instruction stream for plain and flagged pairs (a fixed cell's values are computed and dropped)
                 collide_bgk<Q, FORCE, SC>(f[0], p);
                 collide_bgk<Q, FORCE, SC>(f[1], p);
-#pragma unroll
-                for (int i = 0; i < Q; ++i) {
-                    if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
-                    else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PC::enc2(f[0][i], f[1][i], tab);
-                }
-            } else if (slow) {
-                // f holds every direction pulled from the stage as if there were no wall.  Cell by cell: fixed cells are
-                // not written (R15); a cell next to a wall replaces its bounced links (R3, R9).
-#pragma unroll
-                for (int j = 0; j < 2; ++j)                                     // all bounced loads of both cells first
-                    if (bm[j]) bounce_links<Q, F, SC>(A, p, own + j, c.x0 + xl + j, y, z, bm[j], f[j]);
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    if ((fl >> (8 * j)) & FLAG_FIXED) continue;
-                    const long long n = own + j;
-                    collide_bgk<Q, FORCE, SC>(f[j], p);
+                T *o = B + own;
+                if (!slow) {
 #pragma unroll
                     for (int i = 0; i < Q; ++i) {
-                        if constexpr (ES == 4) B[(long long)i * p.N + n] = f[j][i];
-                        else B[(long long)i * p.N + n] = (T)PC::enc1(f[j][i], tab);
+                        if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + (long long)i * p.N) = make_float2(f[0][i], f[1][i]);
+                        else *reinterpret_cast<unsigned *>(o + (long long)i * p.N) = PC::enc2(f[0][i], f[1][i], tab);
+                    }
+                } else {
+                    // fixed cells (wall, equilibrium boundary) are not written: PAPER.md:1017; R15
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        if ((fl >> (8 * j)) & FLAG_FIXED) continue;
+#pragma unroll
+                        for (int i = 0; i < Q; ++i) {
+                            if constexpr (ES == 4) o[(long long)i * p.N + j] = f[j][i];
+                            else o[(long long)i * p.N + j] = (T)PC::enc1(f[j][i], tab);
+                        }
                     }
                 }
             }
