@@ -91,3 +91,38 @@ def test_read_rho_u_at_equals_full_readout():
         with pytest.raises(lbm.LbmError):
             s.read_rho_u_at([w.n_cells])
         s.close()
+
+
+def test_no_write_outside_the_bound_ddf_buffers():
+    """compute-sanitizer is closed on this pool: the DDF buffers are bound inside a larger tensor filled with a
+    canary pattern, and the canaries must survive init, steps and read-out of both kernels on ragged shapes."""
+    import ctypes as C
+
+    import torch
+
+    import workloads as wl
+    L = lbm.lib()
+    guard = 1 << 16
+    for q, shape in ((19, (48, 5, 3)), (19, (1040, 2, 2)), (27, (32, 3, 3)), (9, (64, 7, 1)), (19, (37, 3, 2))):
+        w = wl.perturbed_equilibrium(*shape, seed=8, velset=q)
+        w = wl.random_walls(w, 0.1, seed=3, moving_fraction=0.5)
+        for name in ("FP32", "FP16S", "P16_2C"):
+            for variant in (2 if shape[0] % 2 == 0 else 1, lbm.VARIANT_BULK):
+                if variant == lbm.VARIANT_BULK and shape[0] % 16:
+                    continue
+                nb = lbm.ddf_buffer_bytes(*shape, q, name)
+                big = torch.full((2 * nb + 3 * guard,), 0xA5, dtype=torch.uint8, device="cuda")
+                a = big.data_ptr() + guard
+                b = a + nb + guard
+                assert a % 16 == 0 and b % 16 == 0
+                s = lbm.Simulation(*shape, q, name, w.tau, use_torch_memory=False)
+                assert L.lbm_bind(s._h, a, b, torch.cuda.current_stream().cuda_stream) == 0
+                s.set_variant(variant)
+                s.set_flags(w.flags)
+                s.init(w.rho, w.u)
+                s.step(5)
+                s.read_rho_u()
+                s.close()
+                torch.cuda.synchronize()
+                canary = torch.cat([big[:guard], big[guard + nb:2 * guard + nb], big[2 * guard + 2 * nb:]])
+                assert bool((canary == 0xA5).all()), (q, shape, name, variant)
