@@ -111,11 +111,15 @@ struct BulkShape {
     static constexpr int PAD = 16;                      // halo pad in front of and behind every segment
     static constexpr int MAXB = (227 * 1024 - 2048) / 2;                    // two CTAs per SM
     static constexpr int TABB = PairCodec<F>::TABLE ? 512 * 16 : 0;        // the format's encoder table
-    static constexpr int row_stage(int r) { return Q * r * (TX * ES + 2 * PAD) + r * TX; }
-    static constexpr int RMAX = 2 * row_stage(2) + TABB <= MAXB ? 2 : 1;    // full-width rows per tile
     static constexpr int PITCH = TX * ES + 2 * PAD;                         // row pitch when rows are copied one by one
-    static constexpr int ROWB = RMAX * PITCH;                               // one direction of one stage
-    static constexpr int STAGEB = row_stage(RMAX);                          // + the tile's flag bytes
+    // bytes of a stage of r full-width rows; rows copied one by one need pads per row, contiguous rows one pair
+    static constexpr int row_stage(int r, bool padded) { return Q * (padded ? r * PITCH : r * TX * ES + 2 * PAD) + r * TX; }
+    static constexpr bool FIT2P = 2 * row_stage(2, true) + TABB <= MAXB, FIT2U = 2 * row_stage(2, false) + TABB <= MAXB;
+    static constexpr int RMAX = (FIT2P || FIT2U) ? 2 : 1;                   // full-width rows per stage
+    static constexpr bool PADDED = RMAX == 1 || FIT2P;
+    static constexpr int RMULTI = PADDED ? RMAX : 1;                        // rows per tile when a row spans several tiles
+    static constexpr int ROWB = PADDED ? RMAX * PITCH : RMAX * TX * ES + 2 * PAD;   // one direction of one stage
+    static constexpr int STAGEB = row_stage(RMAX, PADDED);                  // + the tile's flag bytes
     static constexpr int S = 3 * STAGEB + TABB <= MAXB ? 3 : 2;             // input stages
     static constexpr int TAB_OFF = S * STAGEB;
     static constexpr int BAR_OFF = TAB_OFF + TABB;
