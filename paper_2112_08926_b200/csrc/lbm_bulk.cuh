@@ -9,11 +9,11 @@
 // memory every address is "thread base + compile-time immediate".
 //
 // Shape of the kernel
-//   * persistent CTAs (grid = SMs x resident CTAs), tiles handed out round-robin.  A tile is up to TX = 2*NT
-//     consecutive cells of one row (y, z); when a row is a single tile (nx <= TX) a tile is up to RMAX
-//     consecutive rows of one z-plane: in the SoA layout they are ONE contiguous segment per direction, so the
-//     number of copies per cell and all per-tile bookkeeping halve.  NT threads, two neighbouring cells each,
-//     row after row;
+//   * persistent CTAs (grid = SMs x resident CTAs, two per SM), tiles handed out round-robin.  A stage holds up to
+//     RMAX*TX cells (TX = 2*NT = 512; RMAX = 1, 2 or 4 by velocity set and element size).  If a row fits (nx <=
+//     RMAX*TX) a tile is as many whole consecutive rows of one z-plane as fit: in the SoA layout they are ONE
+//     contiguous segment per direction, one copy.  Longer rows are cut into segments of RMAX*TX cells.  NT threads,
+//     two neighbouring cells each, pair after pair across the tile;
 //   * every warp issues a share of the copies (one lane issues; the bulk-copy instruction is warp-uniform): warp v
 //     the directions v, v+NW, ... -- the copy of direction i is the segment of source row (y - c_iy, z - c_iz)
 //     (periodic wrap in y and z is just a different row address, R2) -- plus one copy of the tile's flag bytes,
@@ -21,7 +21,7 @@
 //     its values in registers arrives on the stage's "empty" mbarrier; before issuing its share of the refill
 //     (tile k+S) a warp waits for that barrier -- there is no CTA-wide barrier in the loop;
 //   * the x +- 1 shift of 10 of the 19 directions is a shared-memory read at offset +- 1 element; the
-//     periodic wrap in x reads the other end of the same row when the tile spans the row, else a 16-byte
+//     periodic wrap in x reads the other end of the same row when the tile holds whole rows, else a 16-byte
 //     halo copy per shifted direction fills the pad in front of / behind the segment;
 //   * results are encoded in registers and stored directly (one aligned 32/64-bit store per direction and cell
 //     pair, 128/256 contiguous bytes per warp): stores need no latency hiding, so they need no staging;
@@ -51,9 +51,9 @@ struct FastDiv {
 };
 
 struct BulkGeom {
-    int tile_w;            // cells of a full tile row: nx if a whole row fits a stage (nx <= RMAX*TX), else TX
+    int tile_w;            // cells of a full tile row: min(nx, RMAX*TX)
     int tiles_per_row;     // ceil(nx / tile_w)
-    int rows_per_tile;     // rows of a tile: RMAX*TX / nx if a row is one tile (their segments are contiguous), else RMAX
+    int rows_per_tile;     // RMAX*TX / nx whole rows if a row is one tile (they are contiguous in memory), else 1
     int ytiles;            // ceil(ny / rows_per_tile)
     int n_tiles;           // tiles_per_row * ytiles * nz  (< 2^31)
     FastDiv by_tpr, by_ytiles;
@@ -111,15 +111,12 @@ struct BulkShape {
     static constexpr int PAD = 16;                      // halo pad in front of and behind every segment
     static constexpr int MAXB = (227 * 1024 - 2048) / 2;                    // two CTAs per SM
     static constexpr int TABB = PairCodec<F>::TABLE ? 512 * 16 : 0;        // the format's encoder table
-    static constexpr int PITCH = TX * ES + 2 * PAD;                         // row pitch when rows are copied one by one
-    // bytes of a stage of r full-width rows; rows copied one by one need pads per row, contiguous rows one pair
-    static constexpr int row_stage(int r, bool padded) { return Q * (padded ? r * PITCH : r * TX * ES + 2 * PAD) + r * TX; }
-    static constexpr bool FIT2P = 2 * row_stage(2, true) + TABB <= MAXB, FIT2U = 2 * row_stage(2, false) + TABB <= MAXB;
-    static constexpr int RMAX = (FIT2P || FIT2U) ? 2 : 1;                   // full-width rows per stage
-    static constexpr bool PADDED = RMAX == 1 || FIT2P;
-    static constexpr int RMULTI = PADDED ? RMAX : 1;                        // rows per tile when a row spans several tiles
-    static constexpr int ROWB = PADDED ? RMAX * PITCH : RMAX * TX * ES + 2 * PAD;   // one direction of one stage
-    static constexpr int STAGEB = row_stage(RMAX, PADDED);                  // + the tile's flag bytes
+    // a stage holds up to RMAX*TX cells of every direction -- several whole rows (contiguous in memory) or one segment
+    // of a long row -- between one pair of pads, plus their flag bytes
+    static constexpr int stage_bytes(int r) { return Q * (r * TX * ES + 2 * PAD) + r * TX; }
+    static constexpr int RMAX = 2 * stage_bytes(4) + TABB <= MAXB ? 4 : 2 * stage_bytes(2) + TABB <= MAXB ? 2 : 1;
+    static constexpr int ROWB = RMAX * TX * ES + 2 * PAD;                   // one direction of one stage
+    static constexpr int STAGEB = stage_bytes(RMAX);
     static constexpr int S = 3 * STAGEB + TABB <= MAXB ? 3 : 2;             // input stages
     static constexpr int TAB_OFF = S * STAGEB;
     static constexpr int BAR_OFF = TAB_OFF + TABB;
@@ -214,9 +211,9 @@ __device__ __forceinline__ void issue_tile_loads(const typename Elem<F>::T *__re
     const bool single = g.tiles_per_row == 1;
     const TileCoord c = tile_coord(t, g, p);
     const int cells = c.rows * c.w;
-    // single: the rows of the tile are one contiguous segment per direction (pitch = w elements); else every row
-    // is copied on its own, with its own halo pads (pitch = SH::PITCH bytes)
-    const int pitch = single ? c.w * ES : SH::PITCH;
+    // single: the rows of the tile are one contiguous segment per direction; else the tile is part of one row and
+    // the shifted directions get a 16-byte halo copy
+    const int pitch = c.w * ES;
     if (warp == 0)
         mbar_arrive_expect_tx(full, (unsigned)(Q * cells * ES + cells + (single ? 0 : c.rows * n_shift * SH::PAD)));
     const long long own = (long long)p.nx * (c.y + (long long)p.ny * c.z);
@@ -353,7 +350,7 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
         const TileCoord c = tile_coord(t, g, p);
         const int w = c.w, hw = w >> 1;
         const char *stage = smem + s * SH::STAGEB;
-        const int pitch = single ? w * ES : SH::PITCH;
+        const int pitch = w * ES;
         const int pairs = c.rows * hw;                                          // cell pairs of the tile
         const FastDiv by_hw = c.last ? g.by_hw_last : g.by_hw_full;
 

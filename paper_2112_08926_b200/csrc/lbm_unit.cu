@@ -40,9 +40,9 @@ constexpr int BULK_NT = 256;
 BulkGeom bulk_geom(const Params &p, long long *tiles) {
     typedef BulkShape<Q, F, BULK_NT> SH;
     BulkGeom g;
-    g.tile_w = p.nx <= SH::RMAX * SH::TX ? p.nx : SH::TX;
+    g.tile_w = p.nx <= SH::RMAX * SH::TX ? p.nx : SH::RMAX * SH::TX;
     g.tiles_per_row = (p.nx + g.tile_w - 1) / g.tile_w;
-    g.rows_per_tile = g.tiles_per_row == 1 ? SH::RMAX * SH::TX / p.nx : SH::RMULTI;
+    g.rows_per_tile = g.tiles_per_row == 1 ? SH::RMAX * SH::TX / p.nx : 1;
     const int w_last = p.nx - (g.tiles_per_row - 1) * g.tile_w;
     g.by_hw_full = FastDiv::make(g.tile_w / 2);
     g.by_hw_last = FastDiv::make(w_last / 2);
