@@ -356,7 +356,10 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
 
         mbar_wait(bar_full + s * 8, ph);
 #pragma unroll 1
-        for (int it = 0, fp = tid; it * NT < pairs; ++it, fp += NT) {           // same trip count for every thread
+        // the pairs of a tile rotate through the warps from tile to tile: a pair that is always slow (row ends next to
+        // walls) does not always burden the same warp
+        const int tidr = (tid + 32 * (k % NW)) & (NT - 1);
+        for (int it = 0, fp = tidr; it * NT < pairs; ++it, fp += NT) {          // same trip count for every thread
             const bool active = fp < pairs;
             const int r = hw == NT ? it : by_hw.div(fp);                        // row of the tile holding this cell pair
             const int xl = 2 * (fp - r * hw);
