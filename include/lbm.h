@@ -10,8 +10,8 @@
  *   - every function returns an int status: LBM_OK (0) or a negative LBM_E_* code; no C++ exception
  *     crosses the boundary; lbm_last_error() gives a thread-local human-readable message.
  *   - cell index n = x + nx*(y + ny*z); N = nx*ny*nz.
- *   - DDF buffers are structure-of-arrays [q][N], element = float (LBM_FP32) or
- *     uint16 (all other formats); the library keeps two of them (A-B / one-step pull).
+ *   - DDF buffers are structure-of-arrays [q][N], element = float (LBM_FP32, LBM_FP64_FP32),
+ *     double (LBM_FP64) or uint16 (all other formats); the library keeps two of them (A-B / one-step pull).
  *     The stored quantity is the SHIFTED DDF f_i - w_i.
  *   - rho is float [N]; u is float [3][N] (ux | uy | uz).
  *   - flags are 1 byte per cell; bit LBM_FLAG_WALL (TYPE_W) marks a halfway
@@ -44,7 +44,14 @@ enum {
     LBM_P16_0S = 3, /* posit<16,0>, sign-magnitude, scaled by 2^7      */
     LBM_P16_1S = 4, /* posit<16,1>, sign-magnitude, scaled by 2^7  */
     LBM_P16_2C = 5, /* one-sided regime, 2 exponent bits, unscaled */
-    LBM_FP16 = 6    /* plain IEEE binary16 (Table 2 row 139)                          */
+    LBM_FP16 = 6,   /* plain IEEE binary16 (Table 2 row 139)                          */
+    /* The two formats below also switch the ARITHMETIC to IEEE binary64 (the paper's "FP64/FP64" and "FP64/FP32"
+     * columns, arithmetic / storage; Tables 3-5): same path, same operation order,
+     * omega = 1 / (double)tau, weights and 1/sqrt(3) in double.  rho, u, force and the wall velocity stay float at
+     * this boundary and are widened exactly; lbm_read_rho_u rounds the double results to float,
+     * lbm_read_rho_u_f64 returns them unrounded. */
+    LBM_FP64 = 7,     /* element = double, identity load/store                                      */
+    LBM_FP64_FP32 = 8 /* element = float: load widens, store rounds to nearest even                 */
 };
 /* LBM_FLAG_WALL: halfway bounce-back wall cell (TYPE_W), optionally moving (its u).
  * LBM_FLAG_EQ:   equilibrium boundary cell (TYPE_E; "equilibrium boundaries"; R15): it keeps
@@ -106,12 +113,15 @@ int lbm_step(lbm_t *h, int n);
  * lbm_read_rho_u: HOST pointers, synchronises.  lbm_read_rho_u_device: DEVICE pointers, asynchronous. */
 int lbm_read_rho_u(lbm_t *h, float *rho, float *u);
 int lbm_read_rho_u_device(lbm_t *h, float *rho_dev, float *u_dev);
+/* The same read-out in double, for the FP64-arithmetic formats (LBM_FP64, LBM_FP64_FP32; LBM_E_UNSUPPORTED for the
+ * others): rho = HOST N doubles, u = HOST 3N doubles, either may be NULL.  Synchronises. */
+int lbm_read_rho_u_f64(lbm_t *h, double *rho, double *u);
 
 /* The same read-out at `count` selected cells (probes of a long run): cells = HOST array of cell indices n,
  * rho = HOST count floats, u = HOST 3*count floats (ux of all probes | uy | uz).  Synchronises. */
 int lbm_read_rho_u_at(lbm_t *h, const long long *cells, int count, float *rho, float *u);
 
-/* Copy direction i (0 <= i < q) of the current DDF buffer, as stored (N elements of 2 or 4 bytes),
+/* Copy direction i (0 <= i < q) of the current DDF buffer, as stored (N elements of 2, 4 or 8 bytes),
  * to a HOST pointer.  Synchronises.  For bit-level parity tests. */
 int lbm_read_ddf(lbm_t *h, int i, void *out);
 

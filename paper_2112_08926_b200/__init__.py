@@ -25,7 +25,8 @@ LIB_PATH = os.path.join(HERE, "liblbm_b200.so")
 
 D2Q9, D3Q19, D3Q27 = 9, 19, 27
 BGK, TRT = 0, 1
-FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C": 5, "FP16": 6}
+FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C": 5, "FP16": 6,
+           "FP64": 7, "FP64_FP32": 8}     # 7, 8: FP64 arithmetic with double / float storage
 FORMAT_NAMES = {v: k for k, v in FORMATS.items()}
 FLAG_WALL, FLAG_EQ = 0x01, 0x02
 VARIANT_AUTO, VARIANT_BULK = 0, 16
@@ -44,6 +45,7 @@ SYMBOLS = {
     "lbm_step": (_i, [_p, _i]),
     "lbm_read_rho_u": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_device": (_i, [_p, _p, _p]),
+    "lbm_read_rho_u_f64": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_at": (_i, [_p, _p, _i, _p, _p]),
     "lbm_read_ddf": (_i, [_p, _i, _p]),
     "lbm_sync": (_i, [_p]),
@@ -215,6 +217,13 @@ class Simulation:
         _check(lib().lbm_read_rho_u(self._h, _np_ptr(rho), _np_ptr(u)))
         return rho, u
 
+    def read_rho_u_f64(self):
+        """Host read-out in double (FP64-arithmetic formats only): (rho [N], u [3, N]) float64."""
+        rho = np.empty(self.N, np.float64)
+        u = np.empty((3, self.N), np.float64)
+        _check(lib().lbm_read_rho_u_f64(self._h, _np_ptr(rho), _np_ptr(u)))
+        return rho, u
+
     def read_rho_u_device(self):
         import torch
         rho = torch.empty(self.N, dtype=torch.float32, device="cuda")
@@ -231,7 +240,7 @@ class Simulation:
         return rho, u
 
     def read_ddf(self, i: int) -> np.ndarray:
-        out = np.empty(self.N, np.float32 if self.fmt == 0 else np.uint16)
+        out = np.empty(self.N, {0: np.float32, 7: np.float64, 8: np.float32}.get(self.fmt, np.uint16))
         _check(lib().lbm_read_ddf(self._h, int(i), _np_ptr(out)))
         return out
 

@@ -28,6 +28,7 @@ FLAGS = ARCH + (["-DLBM_SELFTEST_DEBUG"] if os.environ.get("LBM_SELFTEST_DEBUG")
                 "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-Xptxas", "-v"]
 VELSETS = (9, 19, 27)
 FORMATS = (0, 1, 2, 3, 4, 5, 6)
+FORMATS64 = (7, 8)          # FP64 arithmetic: double / float storage (csrc/lbm_unit64.cu)
 HEADERS = ["lbm_codecs.cuh", "lbm_lattice.cuh", "lbm_kernels.cuh", "lbm_internal.h"]
 
 
@@ -36,6 +37,9 @@ def _jobs():
     for q in VELSETS:
         for f in FORMATS:
             jobs.append((os.path.join(CSRC, "lbm_unit.cu"), os.path.join(OBJ, f"unit_q{q}_f{f}.o"), [f"-DLBM_Q={q}", f"-DLBM_F={f}"]))
+    for q in VELSETS:
+        for f in FORMATS64:
+            jobs.append((os.path.join(CSRC, "lbm_unit64.cu"), os.path.join(OBJ, f"unit_q{q}_f{f}.o"), [f"-DLBM_Q={q}", f"-DLBM_F={f}"]))
     for name in ("lbm_aux", "lbm_units", "lbm_api"):
         jobs.append((os.path.join(CSRC, name + ".cu"), os.path.join(OBJ, name + ".o"), []))
     return jobs

@@ -58,9 +58,10 @@ int fail(int code, const std::string &msg) {
         }                                                                                               \
     } while (0)
 
-int elem_size(int fmt) { return fmt == LBM_FP32 ? 4 : 2; }
+int elem_size(int fmt) { return fmt == LBM_FP64 ? 8 : (fmt == LBM_FP32 || fmt == LBM_FP64_FP32) ? 4 : 2; }
+bool arith64(int fmt) { return fmt == LBM_FP64 || fmt == LBM_FP64_FP32; }
 bool valid_velset(int v) { return v == LBM_D2Q9 || v == LBM_D3Q19 || v == LBM_D3Q27; }
-bool valid_format(int f) { return f >= LBM_FP32 && f <= LBM_FP16; }
+bool valid_format(int f) { return f >= LBM_FP32 && f <= LBM_FP64_FP32; }
 
 Params make_params(const lbm *h) {
     Params p;
@@ -75,6 +76,7 @@ Params make_params(const lbm *h) {
     p.rho0 = h->rho0;
     p.u0 = h->u0;
     p.bounce = h->bounce;
+    p.tau = h->tau;
     return p;
 }
 
@@ -107,6 +109,7 @@ int ensure_ddf(lbm *h) {
 //   * D2Q9 (9 streams: the staged kernel's per-tile bookkeeping does not pay) and small boxes (L2-resident,
 //     launch-bound): the per-thread kernel, 4 cells per thread for D2Q9, else 2.
 int pick_variant(const lbm *h) {
+    if (arith64(h->fmt)) return 1;            // FP64 arithmetic: one kernel, one cell per thread (lbm_fp64.cuh)
     int want = h->V_request;
     if (want == 0) {
         const char *env = getenv("LBM_VARIANT");
@@ -206,6 +209,7 @@ int lbm_set_variant(lbm_t *h, int v) {
         return fail(LBM_E_INVAL, "lbm_set_variant: 0 (auto), 1, 2, 4 (cells per thread) or LBM_VARIANT_BULK");
     if ((v == 2 || v == 4) && h->nx % v != 0) return fail(LBM_E_INVAL, "lbm_set_variant: nx must be a multiple of the cells per thread");
     if (v == LBM_VARIANT_BULK && h->nx % 16 != 0) return fail(LBM_E_INVAL, "lbm_set_variant: the staged kernel needs nx to be a multiple of 16");
+    if (v == LBM_VARIANT_BULK && arith64(h->fmt)) return fail(LBM_E_UNSUPPORTED, "lbm_set_variant: the FP64-arithmetic formats have no staged kernel");
     h->V_request = v;
     h->V = pick_variant(h);
     if (v == LBM_VARIANT_BULK && h->V != v) return fail(LBM_E_INVAL, "lbm_set_variant: box too large for the staged kernel's tile index");
@@ -326,6 +330,23 @@ int lbm_read_rho_u(lbm_t *h, float *rho, float *u) {
     cudaError_t e = h->ops->read(h->ddf[h->cur], make_params(h), h->has_force, rho ? d : nullptr, u ? d + h->N : nullptr, h->stream);
     if (e == cudaSuccess && rho) e = cudaMemcpyAsync(rho, d, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && u) e = cudaMemcpyAsync(u, d + h->N, (size_t)h->N * 12, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    cudaFree(d);
+    LBM_CUDA_TRY(e);
+    LBM_CUDA_TRY(e2);
+    return LBM_OK;
+}
+
+int lbm_read_rho_u_f64(lbm_t *h, double *rho, double *u) {
+    if (int rc = enter(h)) return rc;
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u_f64: call lbm_init first");
+    if (!h->ops->read64) return fail(LBM_E_UNSUPPORTED, "lbm_read_rho_u_f64: FP64-arithmetic formats only (LBM_FP64, LBM_FP64_FP32)");
+    if (!rho && !u) return LBM_OK;
+    double *d = nullptr;
+    LBM_CUDA_TRY(cudaMalloc((void **)&d, (size_t)h->N * 32));
+    cudaError_t e = h->ops->read64(h->ddf[h->cur], make_params(h), h->has_force, rho ? d : nullptr, u ? d + h->N : nullptr, h->stream);
+    if (e == cudaSuccess && rho) e = cudaMemcpyAsync(rho, d, (size_t)h->N * 8, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess && u) e = cudaMemcpyAsync(u, d + h->N, (size_t)h->N * 24, cudaMemcpyDeviceToHost, h->stream);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
     cudaFree(d);
     LBM_CUDA_TRY(e);

@@ -1,0 +1,249 @@
+// lbm_fp64.cuh -- the stream-collide step with FP64 ARITHMETIC: the paper's FP64/FP64 and FP64/FP32 columns
+// (arithmetic / storage precision; Tables 3-5; "FP64/xx") and the
+// FP64 storage of config 5 of BASELINE.json.
+//
+// Same path as lbm_kernels.cuh (Listing 2; eqs (24)-(28)) and the same
+// readings R1-R12, R15, with every FP32 operation replaced by the IEEE binary64 one in the
+// same order: explicitly rounded intrinsics (never contracted), IEEE division, fma where the paper counts an FMA.
+// Storage S = double (identity load / store) or float (load widens exactly, store rounds to nearest even,
+// PAPER.md:787-790 with the cast of a double).  Weights are the doubles 1/3, 1/18, 1/36, ... (Table 1,
+// PAPER.md:72-77), the clamp constant is 1/sqrt(3) in double.  The init fields, the wall velocity
+// and the body force stay FP32 at the boundary (include/lbm.h) and are widened exactly.
+//
+// One cell per thread: 19 eight-byte streams per warp are 256-byte coalesced segments already, and two cells of
+// doubles per thread would not fit the register file at a useful occupancy.  305 B per cell (FP64/FP64) against
+// about 330 FP64 operations: bound by HBM, not by the FP64 pipe.
+#pragma once
+#include "lbm_lattice.cuh"
+
+namespace lbmk {
+
+struct Params64 {
+    double omega, one_m_omega;      // omega = dt / tau in double, from the float tau of lbm_create
+    double F[3];                    // uniform body force, widened
+    double cs;                      // 1 / sqrt(3)
+};
+
+namespace f64 {
+
+__device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+
+template <int Q>
+__device__ __forceinline__ double wgt(int i) { return Lat<Q>::wd(i); }
+
+// c_i . v, terms in x, y, z order, left to right, zero components skipped (i is a compile-time constant after unrolling)
+template <int Q>
+__device__ __forceinline__ double cdot(int i, double vx, double vy, double vz) {
+    typedef Lat<Q> L;
+    const double v[3] = {vx, vy, vz};
+    double s = 0.0;
+    bool first = true;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (L::c(i, a) == 0) continue;
+        const double term = L::c(i, a) > 0 ? v[a] : -v[a];
+        s = first ? term : add(s, term);
+        first = false;
+    }
+    return s;
+}
+
+// R4: rho = (f0 + f1 + ... + f_{q-1}) + 1, the "+1" last; momentum by the alternating sums
+// of PAPER.md:62, 955-959, left to right
+template <int Q>
+__device__ __forceinline__ void moments(const double (&f)[Q], double &rho, double (&j)[3]) {
+    typedef Lat<Q> L;
+    double sum = f[0];
+#pragma unroll
+    for (int i = 1; i < Q; ++i) sum = add(sum, f[i]);
+    rho = add(sum, 1.0);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        double s = 0.0;
+        bool first = true;
+#pragma unroll
+        for (int i = 1; i < Q; i += 2) {
+            if (L::c(i, a) == 0) continue;
+            const int p = L::c(i, a) > 0 ? i : i + 1, m = L::c(i, a) > 0 ? i + 1 : i;
+            s = first ? f[p] : add(s, f[p]);
+            s = sub(s, f[m]);
+            first = false;
+        }
+        j[a] = s;
+    }
+}
+
+// R7: shifted equilibrium, eq (3): three FMAs per direction
+template <int Q>
+__device__ __forceinline__ void equilibrium(double rho, double ux, double uy, double uz, double (&feq)[Q]) {
+    const double c3 = mul(-3.0, add(add(mul(ux, ux), mul(uy, uy)), mul(uz, uz)));
+    const double rhom1 = sub(rho, 1.0);
+    ux = mul(ux, 3.0);
+    uy = mul(uy, 3.0);
+    uz = mul(uz, 3.0);
+    feq[0] = fma_(mul(wgt<Q>(0), rho), mul(0.5, c3), mul(wgt<Q>(0), rhom1));
+#pragma unroll
+    for (int i = 1; i < Q; i += 2) {
+        const double A = mul(wgt<Q>(i), rho), D = mul(wgt<Q>(i), rhom1);
+        const double B = cdot<Q>(i, ux, uy, uz);
+        const double t = fma_(B, B, c3);
+        feq[i] = fma_(A, fma_(0.5, t, B), D);
+        feq[i + 1] = fma_(A, fma_(0.5, t, -B), D);
+    }
+}
+
+// R4 moments, R5 velocity (+ F/2), R6 clamp, R7 equilibrium, R8 BGK (eq (28)), R10 Guo source
+template <int Q, bool FORCE>
+__device__ __forceinline__ void collide_bgk(double (&f)[Q], const Params64 &d) {
+    double rho, j[3], u[3];
+    moments<Q>(f, rho, j);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double ja = FORCE ? fma_(0.5, d.F[a], j[a]) : j[a];
+        u[a] = __ddiv_rn(ja, rho);
+        u[a] = fmin(fmax(u[a], -d.cs), d.cs);
+    }
+    double feq[Q];
+    equilibrium<Q>(rho, u[0], u[1], u[2], feq);
+    double uF = 0.0;
+    if (FORCE) uF = add(add(mul(u[0], d.F[0]), mul(u[1], d.F[1])), mul(u[2], d.F[2]));
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+        double out = fma_(d.one_m_omega, f[i], mul(d.omega, feq[i]));
+        if (FORCE) {
+            const double pref = mul(sub(1.0, mul(0.5, d.omega)), wgt<Q>(i));
+            const double cu = i == 0 ? 0.0 : cdot<Q>(i, u[0], u[1], u[2]);
+            const double cF = i == 0 ? 0.0 : cdot<Q>(i, d.F[0], d.F[1], d.F[2]);
+            out = add(out, mul(pref, fma_(mul(9.0, cu), cF, mul(3.0, sub(cF, uF)))));
+        }
+        f[i] = out;
+    }
+}
+
+template <class S>
+__device__ __forceinline__ double ld(const S *p) { return (double)__ldg(p); }
+template <class S>
+__device__ __forceinline__ void st(S *p, double x) { *p = (S)x; }      // float: cvt.rn.f32.f64
+
+constexpr int THREADS = 256;
+
+// grid: x = tiles of BX cells along x, y = tiles of BY rows, z = plane; blockDim = (BX, BY), BX * BY = THREADS
+template <int Q, class S, bool FORCE>
+__global__ void __launch_bounds__(THREADS)
+stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params p, const Params64 d) {
+    typedef Lat<Q> L;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= p.nx || y >= p.ny) return;
+
+    // R2: periodic neighbours without modulo
+    const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
+    const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
+    const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
+    long long rows[3][3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
+    const int xs[3] = {x == 0 ? p.nx - 1 : x - 1, x, x == p.nx - 1 ? 0 : x + 1};
+    const long long own = rows[1][1] + x;
+
+    const unsigned flag = __ldg(p.flags + own);                          // a1
+    if (flag & FLAG_FIXED) return;                                       // PAPER.md:1017; R15
+
+    double f[Q];
+    if (!(flag & FLAG_NEAR)) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i)                                      // a2, a3: source cell x - c_i
+            f[i] = ld(A + (long long)i * p.N + rows[1 - L::c(i, 1)][1 - L::c(i, 2)] + xs[1 - L::c(i, 0)]);
+    } else {
+        f[0] = ld(A + own);
+#pragma unroll
+        for (int i = 1; i < Q; ++i) {
+            const long long src = rows[1 - L::c(i, 1)][1 - L::c(i, 2)] + xs[1 - L::c(i, 0)];
+            if (__ldg(p.flags + src) & FLAG_WALL) {                      // R3
+                double v = ld(A + (long long)L::opp(i) * p.N + own);
+                const double uwx = (double)__ldg(p.u0 + src), uwy = (double)__ldg(p.u0 + p.N + src),
+                             uwz = (double)__ldg(p.u0 + 2 * p.N + src);
+                if (uwx != 0.0 || uwy != 0.0 || uwz != 0.0)              // R9, rho_w = 1
+                    v = add(v, mul(6.0 * wgt<Q>(i), cdot<Q>(i, uwx, uwy, uwz)));
+                f[i] = v;
+            } else {
+                f[i] = ld(A + (long long)i * p.N + src);
+            }
+        }
+    }
+    collide_bgk<Q, FORCE>(f, d);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) st(B + (long long)i * p.N + own, f[i]);  // a10
+}
+
+// init: every cell, walls included, both buffers (R11)
+template <int Q, class S>
+__global__ void __launch_bounds__(256)
+init64_kernel(S *__restrict__ A, S *__restrict__ B, const float *__restrict__ rho, const float *__restrict__ u, long long N) {
+    for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
+        double feq[Q];
+        equilibrium<Q>((double)__ldg(rho + n), (double)__ldg(u + n), (double)__ldg(u + N + n), (double)__ldg(u + 2 * N + n), feq);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            st(A + (long long)i * N + n, feq[i]);
+            st(B + (long long)i * N + n, feq[i]);
+        }
+    }
+}
+
+// R12: local moments of cell n of the current buffer; flagged cells return the fields given to init
+template <int Q, class S, bool FORCE>
+__device__ __forceinline__ void cell_rho_u(const S *__restrict__ A, const Params &p, const Params64 &d, long long n, double &rho,
+                                           double (&u)[3]) {
+    const long long N = p.N;
+    if (__ldg(p.flags + n) & FLAG_FIXED) {
+        rho = (double)__ldg(p.rho0 + n);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) u[a] = (double)__ldg(p.u0 + a * N + n);
+    } else {
+        double f[Q], j[3];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) f[i] = ld(A + (long long)i * N + n);
+        moments<Q>(f, rho, j);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) u[a] = __ddiv_rn(FORCE ? fma_(-0.5, d.F[a], j[a]) : j[a], rho);
+    }
+}
+
+// OUT = float (lbm_read_rho_u: the doubles rounded to nearest) or double (lbm_read_rho_u_f64)
+template <int Q, class S, bool FORCE, class OUT>
+__global__ void __launch_bounds__(256)
+read_rho_u64_kernel(const S *__restrict__ A, const Params p, const Params64 d, OUT *__restrict__ rho_out, OUT *__restrict__ u_out) {
+    const long long N = p.N;
+    for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
+        double rho, u[3];
+        cell_rho_u<Q, S, FORCE>(A, p, d, n, rho, u);
+        if (rho_out) rho_out[n] = (OUT)rho;
+        if (u_out) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) u_out[a * N + n] = (OUT)u[a];
+        }
+    }
+}
+
+template <int Q, class S, bool FORCE>
+__global__ void __launch_bounds__(128)
+probe_rho_u64_kernel(const S *__restrict__ A, const Params p, const Params64 d, const long long *__restrict__ cells, int count,
+                     float *__restrict__ rho_out, float *__restrict__ u_out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    double rho, u[3];
+    cell_rho_u<Q, S, FORCE>(A, p, d, cells[k], rho, u);
+    rho_out[k] = (float)rho;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) u_out[a * count + k] = (float)u[a];
+}
+
+}  // namespace f64
+}  // namespace lbmk

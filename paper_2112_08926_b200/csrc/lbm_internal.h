@@ -1,6 +1,7 @@
 // lbm_internal.h -- host-side glue between the C ABI (lbm_api.cu) and the kernel translation units.
 // One translation unit per (velocity set, storage format) pair is compiled from lbm_unit.cu with
-// -DLBM_Q=<q> -DLBM_F=<fmt>; each exports the launchers below under a suffixed name.
+// -DLBM_Q=<q> -DLBM_F=<fmt> (lbm_unit64.cu for the FP64-arithmetic formats 7 and 8); each exports the launchers
+// below under a suffixed name.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -20,6 +21,8 @@ struct UnitOps {
     int (*bulk_tile_cells)();     // cells per tile of the staged kernel
     cudaError_t (*probe)(const void *A, const Params &p, bool force, const long long *cells, int count, float *rho, float *u,
                          cudaStream_t st);
+    // FP64-arithmetic units only (lbm_unit64.cu), else null: read-out in double
+    cudaError_t (*read64)(const void *A, const Params &p, bool force, double *rho, double *u, cudaStream_t st);
 };
 
 const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)
