@@ -319,7 +319,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=512, help="cube edge L")
-    ap.add_argument("--formats", default="FP32,FP16S,FP16C,P16_0S,P16_1S,P16_2C")
+    ap.add_argument("--formats", default="FP32,FP16S,FP16C,P16_0S,P16_1S,P16_2C,FP64,FP64_FP32")
     ap.add_argument("--velset", type=int, default=19, choices=[9, 19, 27], help="sweep only; the headline is D3Q19")
     ap.add_argument("--device-init", action="store_true", help="draw the input on the device (big sweep sizes)")
     ap.add_argument("--cells-per-thread", type=int, default=0, help="0 = library default")

@@ -12,7 +12,8 @@
 //
 // One cell per thread: 19 eight-byte streams per warp are 256-byte coalesced segments already, and two cells of
 // doubles per thread would not fit the register file at a useful occupancy.  305 B per cell (FP64/FP64) against
-// about 330 FP64 operations: bound by HBM, not by the FP64 pipe.
+// 177 FP64 instructions (86 DFMA, 55 DADD, 36 DMUL): bound by HBM, the FP64 pipe is 22% busy.
+// MINB = resident CTAs per SM the register allocation is held to (chosen per storage type by the launcher).
 #pragma once
 #include "lbm_lattice.cuh"
 
@@ -131,8 +132,8 @@ __device__ __forceinline__ void st(S *p, double x) { *p = (S)x; }      // float:
 constexpr int THREADS = 256;
 
 // grid: x = tiles of BX cells along x, y = tiles of BY rows, z = plane; blockDim = (BX, BY), BX * BY = THREADS
-template <int Q, class S, bool FORCE>
-__global__ void __launch_bounds__(THREADS)
+template <int Q, class S, bool FORCE, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
 stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params p, const Params64 d) {
     typedef Lat<Q> L;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -140,31 +141,32 @@ stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params
     const int z = blockIdx.z;
     if (x >= p.nx || y >= p.ny) return;
 
-    // R2: periodic neighbours without modulo
-    const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
-    const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
-    const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
-    long long rows[3][3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
-    const int xs[3] = {x == 0 ? p.nx - 1 : x - 1, x, x == p.nx - 1 ? 0 : x + 1};
-    const long long own = rows[1][1] + x;
+    // R2: periodic neighbours without modulo.  Pull sources are addressed relative to the own cell (in-plane offsets
+    // in 32 bits, the plane offset in 64) and the direction's base walks by N elements, instead of q absolute
+    // 64-bit element indices.
+    const int dyv[3] = {y == 0 ? p.ny - 1 : -1, 0, y == p.ny - 1 ? 1 - p.ny : 1};            // rows to y-1, y, y+1
+    const long long plane = (long long)p.nx * p.ny;
+    const long long dzv[3] = {z == 0 ? plane * (p.nz - 1) : -plane, 0, z == p.nz - 1 ? -plane * (p.nz - 1) : plane};
+    const int dxv[3] = {x == 0 ? p.nx - 1 : -1, 0, x == p.nx - 1 ? 1 - p.nx : 1};
+    const long long own = (long long)p.nx * (y + (long long)p.ny * z) + x;
 
     const unsigned flag = __ldg(p.flags + own);                          // a1
     if (flag & FLAG_FIXED) return;                                       // PAPER.md:1017; R15
 
     double f[Q];
     if (!(flag & FLAG_NEAR)) {
+        const S *Ai = A + own;
 #pragma unroll
-        for (int i = 0; i < Q; ++i)                                      // a2, a3: source cell x - c_i
-            f[i] = ld(A + (long long)i * p.N + rows[1 - L::c(i, 1)][1 - L::c(i, 2)] + xs[1 - L::c(i, 0)]);
+        for (int i = 0; i < Q; ++i) {                                    // a2, a3: source cell x - c_i
+            const long long off = dzv[1 - L::c(i, 2)] + (dyv[1 - L::c(i, 1)] * p.nx + dxv[1 - L::c(i, 0)]);
+            f[i] = ld(Ai + off);
+            Ai += p.N;
+        }
     } else {
         f[0] = ld(A + own);
 #pragma unroll
         for (int i = 1; i < Q; ++i) {
-            const long long src = rows[1 - L::c(i, 1)][1 - L::c(i, 2)] + xs[1 - L::c(i, 0)];
+            const long long src = own + dzv[1 - L::c(i, 2)] + (dyv[1 - L::c(i, 1)] * p.nx + dxv[1 - L::c(i, 0)]);
             if (__ldg(p.flags + src) & FLAG_WALL) {                      // R3
                 double v = ld(A + (long long)L::opp(i) * p.N + own);
                 const double uwx = (double)__ldg(p.u0 + src), uwy = (double)__ldg(p.u0 + p.N + src),
@@ -178,8 +180,12 @@ stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params
         }
     }
     collide_bgk<Q, FORCE>(f, d);
+    S *Bi = B + own;
 #pragma unroll
-    for (int i = 0; i < Q; ++i) st(B + (long long)i * p.N + own, f[i]);  // a10
+    for (int i = 0; i < Q; ++i) {                                        // a10
+        st(Bi, f[i]);
+        Bi += p.N;
+    }
 }
 
 // init: every cell, walls included, both buffers (R11)

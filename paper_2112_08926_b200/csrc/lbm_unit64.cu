@@ -46,7 +46,11 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
     const int by = THREADS / bx;
     const dim3 block(bx, by, 1);
     const dim3 grid((p.nx + bx - 1) / bx, (p.ny + by - 1) / by, p.nz);
-    stream_collide64_kernel<Q, S, FORCE><<<grid, block, 0, st>>>((const S *)A, (S *)B, p, make64(p));
+    // resident CTAs per SM asked of the compiler (measured on 512^3 / 384^3): three (<= 80
+    // registers) for double storage, where the kernel then runs at the HBM roofline; four (<= 64 registers, 28 bytes
+    // of spills) for D2Q9 / D3Q19 float storage, which is bound by latency, not by bytes: 0.76 -> 0.83 of peak
+    constexpr int MINB = (sizeof(S) == 4 && Q <= 19) ? 4 : 3;
+    stream_collide64_kernel<Q, S, FORCE, MINB><<<grid, block, 0, st>>>((const S *)A, (S *)B, p, make64(p));
     count_launch();
     return cudaGetLastError();
 }

@@ -37,6 +37,8 @@ def test_size_helpers_need_no_device(library):
     assert lbm.bytes_per_cell(19, "FP16C") == 2 * 19 * 2 + 1
     assert lbm.bytes_per_cell(27, "P16_1S") == 109
     assert lbm.bytes_per_cell(5, "FP32") == -1
+    assert lbm.bytes_per_cell(19, "FP64") == 305 and lbm.bytes_per_cell(19, "FP64_FP32") == 153
+    assert lbm.ddf_buffer_bytes(8, 8, 4, 27, "FP64") == 8 * 8 * 4 * 27 * 8
     assert lbm.ddf_buffer_bytes(3, 3, 3, 19, "FP32") % 256 == 0
     assert lbm.launch_count() == 0
 

@@ -394,3 +394,26 @@ def test_storage_formats_track_fp64_on_taylor_green():
     for name in wl.FORMATS_16BIT:
         assert err["FP32"] < err[name] < 2e-2, (name, err)
     assert err["FP16C"] < err["FP16S"]                               # one more mantissa bit
+
+
+def test_fp64_arithmetic_with_fp32_storage_mode():
+    """The paper's FP64/FP32 column (arithmetic / storage): the oracle's arith = F64, fmt = FP32
+    mode is the FP64 step with one rounding to float per stored DDF.  Pins: (a) after init its stored DDFs are exactly
+    the FP64/FP64 ones rounded to nearest float; (b) over a run it stays closer to
+    FP64/FP64 than FP32/FP32 does (FP32 arithmetic adds its own rounding, Fig. 8) and mass is conserved to the
+    storage rounding."""
+    w = wl.taylor_green_3d(16)
+    ref = sim64(w)
+    mix = oracle.from_workload(w, oracle.FP32, F64)
+    f32 = oracle.from_workload(w, oracle.FP32)
+    for i in range(19):
+        assert np.array_equal(mix.read_ddf(i), ref.read_ddf(i).astype(np.float32))
+    m0 = mix.sum_ddf()
+    ref.step(40); mix.step(40); f32.step(40)
+    _, uref = ref.read_rho_u(f64=True)
+    _, umix = mix.read_rho_u(f64=True)
+    _, u32 = f32.read_rho_u()
+    e_mix = np.abs(umix - uref).max() / np.abs(uref).max()
+    e_32 = np.abs(u32 - uref).max() / np.abs(uref).max()
+    assert e_mix < 1e-6 and e_mix <= e_32
+    assert abs(mix.sum_ddf() - m0) < 40 * 19 * 16 ** 3 * 2.0 ** -36      # each store rounds |f| < 2^-11 to 2^-36 at worst
