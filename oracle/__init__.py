@@ -15,6 +15,7 @@ from . import build as _build
 
 FP32, FP16S, FP16C, P16_0S, P16_1S, P16_2C, FP16, FP64 = range(8)
 ARITH_F32, ARITH_F64 = 0, 1
+BGK, TRT = 0, 1
 
 _lib = None
 
@@ -34,6 +35,7 @@ def lib():
         L.orc_create.argtypes = [C.c_int] * 6 + [C.c_double, C.c_void_p]
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_destroy.restype = None
+        L.orc_set_collision.argtypes = [C.c_void_p, C.c_int, C.c_double]
         for name in ("orc_set_flags",):
             getattr(L, name).argtypes = [C.c_void_p, C.c_void_p]
         for name in ("orc_init", "orc_init_f64", "orc_read_rho_u", "orc_read_rho_u_f64"):
@@ -135,6 +137,9 @@ class Sim:
             u = np.ascontiguousarray(u, dtype=np.float32)
             assert rho.size == self.N and u.size == 3 * self.N
             assert lib().orc_init(self._h, _ptr(rho), _ptr(u)) == 0
+
+    def set_collision(self, collision, lam=3.0 / 16.0):
+        assert lib().orc_set_collision(self._h, int(collision), float(lam)) == 0
 
     def step(self, n=1):
         assert lib().orc_step(self._h, int(n)) == 0

@@ -154,6 +154,8 @@ void moments(const VelSet &vs, const T *f, T &rho, T j[3]) {
 
 struct orc_sim {
     int nx, ny, nz, fmt, arith;
+    int collision;                    // ORC_BGK / ORC_TRT
+    double lambda;                    // TRT magic parameter (R13)
     long N;
     VelSet vs;
     double tau;
@@ -220,6 +222,8 @@ void step_t(orc_sim *s) {
     const int A = s->cur, Bb = 1 - s->cur;
     const T omega = T(1) / (T)s->tau;                     // R8: omega = dt / tau
     const T one_m_omega = T(1) - omega;
+    // TRT (R13): omega- from the magic parameter, 1/omega- = 1/2 + Lambda / (tau - 1/2)
+    const T omega_m = T(1) / (T(0.5) + (T)s->lambda / ((T)s->tau - T(0.5)));
     const T cs = sizeof(T) == 4 ? (T)0.57735027f : (T)(1.0 / std::sqrt(3.0));   // R6: c = 1/sqrt(3)
     const T F[3] = {(T)s->force[0], (T)s->force[1], (T)s->force[2]};
     const bool forced = s->has_force;
@@ -262,6 +266,38 @@ void step_t(orc_sim *s) {
                 equilibrium<T>(vs, rho, u[0], u[1], u[2], feq);       // R7
                 T uF = T(0);
                 if (forced) uF = u[0] * F[0] + u[1] * F[1] + u[2] * F[2];
+                if (s->collision == ORC_TRT) {
+                    // R13 (NOT in the paper, which only names TRT): two-relaxation-time collision
+                    // (Ginzburg et al.): per opposite pair (i, i') the symmetric part (f_i + f_i')/2 relaxes with
+                    // omega+ = dt/tau, the antisymmetric part (f_i - f_i')/2 with omega-, where
+                    // Lambda = (1/omega+ - 1/2)(1/omega- - 1/2); the rest DDF has no antisymmetric part.  The Guo
+                    // source splits the same way: symmetric w (9 (c.u)(c.F) - 3 u.F) with (1 - omega+/2),
+                    // antisymmetric 3 w c.F with (1 - omega-/2).
+                    const T gp = T(1) - T(0.5) * omega, gm = T(1) - T(0.5) * omega_m;
+                    {
+                        T out = fma_t<T>(one_m_omega, fh[0], omega * feq[0]);
+                        if (forced) out = out + (gp * (T)vs.w[0]) * (-(T(3) * uF));
+                        store<T>(s, Bb, 0, n, out);
+                    }
+                    for (int i = 1; i < q; i += 2) {
+                        const T fp = T(0.5) * (fh[i] + fh[i + 1]), fm = T(0.5) * (fh[i] - fh[i + 1]);
+                        const T ep = T(0.5) * (feq[i] + feq[i + 1]), em = T(0.5) * (feq[i] - feq[i + 1]);
+                        const T a = omega * (fp - ep), b = omega_m * (fm - em);
+                        T o1 = (fh[i] - a) - b, o2 = (fh[i + 1] - a) + b;
+                        if (forced) {
+                            const T w = (T)vs.w[i];
+                            const T cu = cdot<T>(vs.c[i], u[0], u[1], u[2]);
+                            const T cF = cdot<T>(vs.c[i], F[0], F[1], F[2]);
+                            const T Sp = (gp * w) * fma_t<T>(T(9) * cu, cF, -(T(3) * uF));
+                            const T Sm = (gm * w) * (T(3) * cF);
+                            o1 = (o1 + Sp) + Sm;
+                            o2 = (o2 + Sp) - Sm;
+                        }
+                        store<T>(s, Bb, i, n, o1);
+                        store<T>(s, Bb, i + 1, n, o2);
+                    }
+                    continue;
+                }
                 for (int i = 0; i < q; ++i) {
                     T out = fma_t<T>(one_m_omega, fh[i], omega * feq[i]);          // R8
                     if (forced) {                                                  // R10
@@ -340,7 +376,16 @@ orc_sim *orc_create(int nx, int ny, int nz, int velset, int fmt, int arith, doub
     }
     s->cur = 0;
     s->steps_done = 0;
+    s->collision = ORC_BGK;
+    s->lambda = 3.0 / 16.0;
     return s;
+}
+
+int orc_set_collision(orc_sim *s, int collision, double lambda) {
+    if (!s || (collision != ORC_BGK && collision != ORC_TRT) || !(lambda > 0.0)) return -1;
+    s->collision = collision;
+    s->lambda = s->arith == ORC_ARITH_F32 ? (double)(float)lambda : lambda;
+    return 0;
 }
 
 void orc_destroy(orc_sim *s) { delete s; }

@@ -417,3 +417,61 @@ def test_fp64_arithmetic_with_fp32_storage_mode():
     e_32 = np.abs(u32 - uref).max() / np.abs(uref).max()
     assert e_mix < 1e-6 and e_mix <= e_32
     assert abs(mix.sum_ddf() - m0) < 40 * 19 * 16 ** 3 * 2.0 ** -36      # each store rounds |f| < 2^-11 to 2^-36 at worst
+
+
+# ---- TRT (R13: textbook definition, NOT the paper's -- it only names the operator) --------------
+def test_trt_magic_parameter_removes_the_poiseuille_slip():
+    """With Lambda = 3/16 the halfway bounce-back wall of a force-driven planar channel sits exactly half a cell
+    outside the first fluid node for every tau (Ginzburg & d'Humieres): the steady profile is the plain parabola
+    of eq (9), no slip term -- where BGK has U_s = f (48 nu^2 - 1) / (8 nu) (test_poiseuille_exact_steady_state)."""
+    for tau in (0.8, 1.3):
+        ny, u_max = 18, 0.01
+        w = wl.poiseuille_channel(4, ny, 3, tau=tau, u_max=u_max)
+        nu, H, f = w.meta["nu"], w.meta["H"], w.force[0]
+        s = sim64(w)
+        s.set_collision(oracle.TRT, 3.0 / 16.0)
+        s.step(14000)
+        rho, u = s.read_rho_u(f64=True)
+        prof = u[0].reshape(3, ny, 4)[1, 1:-1, 2]
+        y = np.arange(1, ny - 1) - 0.5
+        assert np.abs(prof - f / (2 * nu) * y * (H - y)).max() / u_max < 1e-10, tau
+        assert np.abs(u[1]).max() < 1e-15 and np.abs(u[2]).max() < 1e-15
+        assert np.abs(rho[w.flags == 0] - 1.0).max() < 1e-12
+
+
+def test_trt_with_equal_rates_is_bgk():
+    """Lambda = (tau - 1/2)^2 makes omega- = omega+: symmetric and antisymmetric parts relax alike, which is BGK
+    (eq (28)), Guo source included -- with walls, moving walls and a force, to FP64 rounding."""
+    tau = 0.7
+    w = wl.random_walls(wl.perturbed_equilibrium(10, 7, 6, seed=2, tau=tau), 0.15, seed=4, moving_fraction=0.5)
+    w.force = (1e-5, -2e-5, 3e-5)
+    a, b = sim64(w), sim64(w)
+    b.set_collision(oracle.TRT, (tau - 0.5) ** 2)
+    a.step(30); b.step(30)
+    for i in range(19):
+        assert np.abs(a.read_ddf(i) - b.read_ddf(i)).max() < 1e-15, i
+
+
+@pytest.mark.parametrize("q,shape", [(19, (8, 6, 5)), (27, (6, 5, 4)), (9, (12, 9, 1))])
+def test_trt_conserves_mass_and_momentum_and_keeps_the_viscosity(q, shape):
+    w = wl.perturbed_equilibrium(*shape, seed=8, velset=q, tau=0.9)
+    s = sim64(w)
+    s.set_collision(oracle.TRT)
+    rho0, u0 = s.read_rho_u(f64=True)
+    s.step(25)
+    rho, u = s.read_rho_u(f64=True)
+    assert abs(rho.sum() - rho0.sum()) < 1e-11
+    assert np.abs((rho * u).sum(1) - (rho0 * u0).sum(1)).max() < 1e-12
+    # the shear viscosity is set by omega+ alone: 2-D Taylor-Green decays as exp(-2 nu k^2 t), as with BGK
+    n, tau = 32, 0.6
+    w = wl.taylor_green_2d(n, n, 1 if q == 9 else 3, u0=0.05, tau=tau, velset=q if q != 27 else 19, with_density=True)
+    s = oracle.Sim(w.nx, w.ny, w.nz, w.velset, oracle.FP64, tau, None, F64)
+    s.set_collision(oracle.TRT)
+    s.init(w.rho.astype(np.float64), w.u.astype(np.float64))
+    s.step(50)
+    _, u50 = s.read_rho_u(f64=True)
+    s.step(150)
+    _, u200 = s.read_rho_u(f64=True)
+    amp = lambda u: (u[0] * w.u[0]).sum() / (w.u[0].astype(np.float64) ** 2).sum()
+    rate = -math.log(amp(u200) / amp(u50)) / 150
+    assert rate == pytest.approx(2 * (tau / 3 - 1 / 6) * (2 * math.pi / n) ** 2, rel=5e-3)
