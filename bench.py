@@ -194,7 +194,8 @@ def run_ours(args):
 
     results, launches_total = {}, 0
     for name in formats:
-        sim = lbm.Simulation(L, L, nz, Q, name, TAU, cells_per_thread=args.cells_per_thread)
+        sim = lbm.Simulation(L, L, nz, Q, name, TAU, cells_per_thread=args.cells_per_thread,
+                             collision=lbm.TRT if args.collision == "TRT" else lbm.BGK)
         sim.init(rho_d, u_d)
         sim.step(W)
         barrier()
@@ -241,7 +242,7 @@ def run_ours(args):
         "metric": METRIC, "value": r["mlups"], "unit": "MLUPs/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"configs[4] bandwidth sweep: D{2 if Q == 9 else 3}Q{Q} BGK periodic {'square' if Q == 9 else 'cube'} {L}^{2 if Q == 9 else 3}, perturbed equilibrium "
+        "config": {"workload": f"configs[4] bandwidth sweep: D{2 if Q == 9 else 3}Q{Q} {args.collision} periodic {'square' if Q == 9 else 'cube'} {L}^{2 if Q == 9 else 3}, perturbed equilibrium "
                                f"(seed {SEED}), tau {TAU}, headline storage format {head}",
                    "cells": N, "l2_policy": "inputs larger than L2 (two DDF buffers of "
                                             f"{N * Q * (4 if head == 'FP32' else 2) / 1e9:.1f} GB each, no flush needed)",
@@ -323,6 +324,7 @@ def main():
     ap.add_argument("--velset", type=int, default=19, choices=[9, 19, 27], help="sweep only; the headline is D3Q19")
     ap.add_argument("--device-init", action="store_true", help="draw the input on the device (big sweep sizes)")
     ap.add_argument("--cells-per-thread", type=int, default=0, help="0 = library default")
+    ap.add_argument("--collision", default="BGK", choices=["BGK", "TRT"], help="sweep only; the headline is BGK (TRT: DESIGN.md R13)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()

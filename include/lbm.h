@@ -34,7 +34,10 @@ typedef struct lbm lbm_t; /* opaque, owned by the library, freed by lbm_destroy 
 /* velocity sets (R1: D3Q19 numbering from PAPER.md:955-959, 1029-1031; D2Q9 needs nz == 1) */
 enum { LBM_D2Q9 = 9, LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
 /* collision operators.  BGK = eq (28).  TRT is named but never
- * defined by the paper: lbm_create answers LBM_E_UNSUPPORTED for LBM_TRT (R13). */
+ * defined by the paper; LBM_TRT is the textbook two-relaxation-time operator (R13): per opposite pair
+ * (i, i') the symmetric part (f_i + f_i')/2 relaxes towards its equilibrium with omega+ = 1/tau, the antisymmetric
+ * part (f_i - f_i')/2 with omega-, where Lambda = (1/omega+ - 1/2)(1/omega- - 1/2) (see lbm_set_trt_lambda); the
+ * Guo source term splits the same way.  Same memory traffic as BGK. */
 enum { LBM_BGK = 0, LBM_TRT = 1 };
 /* DDF storage formats (Table 2, 152-178, 201-219; Listing 1) */
 enum {
@@ -91,6 +94,12 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream);
 enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16 };
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_cells_per_thread(lbm_t *h, int v);
+
+/* LBM_TRT handles only (else LBM_E_STATE): the magic parameter Lambda > 0 (else LBM_E_INVAL), default 3/16 (the
+ * halfway bounce-back wall of a Poiseuille channel then sits exactly half a cell outside the last fluid node).
+ * Lambda = (tau - 1/2)^2 makes omega- = omega+.  The FP32-arithmetic formats use the value rounded to FP32.  May be
+ * called at any time between steps; takes effect from the next lbm_step. */
+int lbm_set_trt_lambda(lbm_t *h, double lambda);
 
 /* Set the cell flags.  flags: HOST pointer, N bytes, copied.  Only LBM_FLAG_WALL or LBM_FLAG_EQ may be set (not both on one cell)
  * (else LBM_E_INVAL).  Must precede lbm_init (LBM_E_STATE otherwise).  Synchronises the stream. */

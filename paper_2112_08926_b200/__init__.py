@@ -38,6 +38,7 @@ SYMBOLS = {
     "lbm_create": (_i, [C.POINTER(_p), _i, _i, _i, _i, _i, _i, _f, _p]),
     "lbm_bind": (_i, [_p, _p, _p, _p]),
     "lbm_set_variant": (_i, [_p, _i]),
+    "lbm_set_trt_lambda": (_i, [_p, C.c_double]),
     "lbm_set_cells_per_thread": (_i, [_p, _i]),
     "lbm_set_flags": (_i, [_p, _p]),
     "lbm_init": (_i, [_p, _p, _p]),
@@ -173,6 +174,9 @@ class Simulation:
     # -- the ABI -------------------------------------------------------------------------------
     def set_cells_per_thread(self, v: int):
         _check(lib().lbm_set_cells_per_thread(self._h, int(v)))
+
+    def set_trt_lambda(self, lam: float):
+        _check(lib().lbm_set_trt_lambda(self._h, float(lam)))
 
     def set_variant(self, v: int):
         _check(lib().lbm_set_variant(self._h, int(v)))

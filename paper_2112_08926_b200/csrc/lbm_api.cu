@@ -21,6 +21,7 @@ struct lbm {
     int nx, ny, nz, q, fmt, collision;
     long long N;
     float tau, omega;
+    double trt_lambda;         // TRT magic parameter Lambda (R13), default 3/16
     float force[3];
     bool has_force;
     int device;
@@ -69,8 +70,10 @@ Params make_params(const lbm *h) {
     p.N = h->N;
     p.omega = h->omega;
     p.one_m_omega = 1.0f - h->omega;
-    p.omega_minus = 0.0f;
-    p.one_m_omega_minus = 0.0f;
+    // R13: Lambda = (1/omega+ - 1/2)(1/omega- - 1/2), evaluated in FP32 like omega
+    p.omega_minus = 1.0f / (0.5f + (float)h->trt_lambda / (h->tau - 0.5f));
+    p.one_m_omega_minus = 1.0f - p.omega_minus;
+    p.trt_lambda = h->trt_lambda;
     p.fx = h->force[0]; p.fy = h->force[1]; p.fz = h->force[2];
     p.flags = h->flags;
     p.rho0 = h->rho0;
@@ -153,8 +156,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, i
     if (!valid_velset(velset)) return fail(LBM_E_INVAL, "lbm_create: velset must be 9, 19 or 27");
     if (velset == LBM_D2Q9 && nz != 1) return fail(LBM_E_INVAL, "lbm_create: D2Q9 needs nz == 1");
     if (!valid_format(ddf_format)) return fail(LBM_E_INVAL, "lbm_create: unknown ddf_format");
-    if (collision == LBM_TRT) return fail(LBM_E_UNSUPPORTED, "lbm_create: TRT is named but not defined by the paper (PAPER.md:43)");
-    if (collision != LBM_BGK) return fail(LBM_E_INVAL, "lbm_create: unknown collision operator");
+    if (collision != LBM_BGK && collision != LBM_TRT) return fail(LBM_E_INVAL, "lbm_create: unknown collision operator");
     if (!(tau > 0.5f)) return fail(LBM_E_INVAL, "lbm_create: tau must be > 0.5 (PAPER.md:79)");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -168,6 +170,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, i
     h->N = (long long)nx * ny * nz;
     h->tau = tau;
     h->omega = 1.0f / tau;
+    h->trt_lambda = 3.0 / 16.0;
     for (int a = 0; a < 3; ++a) {
         h->force[a] = force ? force[a] : 0.0f;
         if (h->force[a] != 0.0f) h->has_force = true;
@@ -213,6 +216,15 @@ int lbm_set_variant(lbm_t *h, int v) {
     h->V_request = v;
     h->V = pick_variant(h);
     if (v == LBM_VARIANT_BULK && h->V != v) return fail(LBM_E_INVAL, "lbm_set_variant: box too large for the staged kernel's tile index");
+    return LBM_OK;
+}
+
+int lbm_set_trt_lambda(lbm_t *h, double lambda) {
+    if (int rc = enter(h)) return rc;
+    if (h->collision != LBM_TRT) return fail(LBM_E_STATE, "lbm_set_trt_lambda: the handle was not created with LBM_TRT");
+    if (!(lambda > 0.0) || !(lambda < 1e30)) return fail(LBM_E_INVAL, "lbm_set_trt_lambda: Lambda must be positive and finite");
+    // FP32 arithmetic sees the FP32 value of Lambda, FP64 arithmetic the double as given
+    h->trt_lambda = arith64(h->fmt) ? lambda : (double)(float)lambda;
     return LBM_OK;
 }
 

@@ -301,7 +301,7 @@ __device__ __forceinline__ void bounce_links(const typename Elem<F>::T *__restri
     }
 }
 
-template <int Q, int F, int NT, bool FORCE>
+template <int Q, int F, int NT, bool FORCE, int COLL = 0>
 __global__ void __launch_bounds__(NT, 2)
 stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p,
                            const BulkGeom g, const EncEntry *__restrict__ enc_table) {
@@ -408,8 +408,8 @@ stream_collide_bulk_kernel(const typename Elem<F>::T *__restrict__ A, typename E
             }
             if (active) {
                 // one instruction stream for plain and flagged pairs (a fixed cell's values are computed and dropped)
-                collide_bgk<Q, FORCE, SC>(f[0], p);
-                collide_bgk<Q, FORCE, SC>(f[1], p);
+                collide<COLL, Q, FORCE, SC>(f[0], p);
+                collide<COLL, Q, FORCE, SC>(f[1], p);
                 T *o = B + own;
                 if (!slow) {
 #pragma unroll

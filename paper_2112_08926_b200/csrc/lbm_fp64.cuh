@@ -21,6 +21,7 @@ namespace lbmk {
 
 struct Params64 {
     double omega, one_m_omega;      // omega = dt / tau in double, from the float tau of lbm_create
+    double omega_minus;             // TRT (R13): 1 / omega- = 1/2 + Lambda / (tau - 1/2)
     double F[3];                    // uniform body force, widened
     double cs;                      // 1 / sqrt(3)
 };
@@ -124,6 +125,45 @@ __device__ __forceinline__ void collide_bgk(double (&f)[Q], const Params64 &d) {
     }
 }
 
+// TRT (R13; NOT defined by the paper, which only names it): as collide_bgk up to the equilibrium,
+// then per opposite pair (i, i + 1) the symmetric part relaxes with omega+, the antisymmetric part with omega-;
+// the Guo source splits the same way.
+template <int Q, bool FORCE>
+__device__ __forceinline__ void collide_trt(double (&f)[Q], const Params64 &d) {
+    double rho, j[3], u[3];
+    moments<Q>(f, rho, j);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double ja = FORCE ? fma_(0.5, d.F[a], j[a]) : j[a];
+        u[a] = __ddiv_rn(ja, rho);
+        u[a] = fmin(fmax(u[a], -d.cs), d.cs);
+    }
+    double feq[Q];
+    equilibrium<Q>(rho, u[0], u[1], u[2], feq);
+    double uF = 0.0;
+    if (FORCE) uF = add(add(mul(u[0], d.F[0]), mul(u[1], d.F[1])), mul(u[2], d.F[2]));
+    const double gp = sub(1.0, mul(0.5, d.omega)), gm = sub(1.0, mul(0.5, d.omega_minus));
+    f[0] = fma_(d.one_m_omega, f[0], mul(d.omega, feq[0]));
+    if (FORCE) f[0] = add(f[0], mul(mul(gp, wgt<Q>(0)), -mul(3.0, uF)));
+#pragma unroll
+    for (int i = 1; i < Q; i += 2) {
+        const double fp = mul(0.5, add(f[i], f[i + 1])), fm = mul(0.5, sub(f[i], f[i + 1]));
+        const double ep = mul(0.5, add(feq[i], feq[i + 1])), em = mul(0.5, sub(feq[i], feq[i + 1]));
+        const double a = mul(d.omega, sub(fp, ep)), b = mul(d.omega_minus, sub(fm, em));
+        double o1 = sub(sub(f[i], a), b), o2 = add(sub(f[i + 1], a), b);
+        if (FORCE) {
+            const double cu = cdot<Q>(i, u[0], u[1], u[2]);
+            const double cF = cdot<Q>(i, d.F[0], d.F[1], d.F[2]);
+            const double Sp = mul(mul(gp, wgt<Q>(i)), fma_(mul(9.0, cu), cF, -mul(3.0, uF)));
+            const double Sm = mul(mul(gm, wgt<Q>(i)), mul(3.0, cF));
+            o1 = add(add(o1, Sp), Sm);
+            o2 = sub(add(o2, Sp), Sm);
+        }
+        f[i] = o1;
+        f[i + 1] = o2;
+    }
+}
+
 template <class S>
 __device__ __forceinline__ double ld(const S *p) { return (double)__ldg(p); }
 template <class S>
@@ -132,7 +172,7 @@ __device__ __forceinline__ void st(S *p, double x) { *p = (S)x; }      // float:
 constexpr int THREADS = 256;
 
 // grid: x = tiles of BX cells along x, y = tiles of BY rows, z = plane; blockDim = (BX, BY), BX * BY = THREADS
-template <int Q, class S, bool FORCE, int MINB>
+template <int Q, class S, bool FORCE, int MINB, int COLL = 0>
 __global__ void __launch_bounds__(THREADS, MINB)
 stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params p, const Params64 d) {
     typedef Lat<Q> L;
@@ -179,7 +219,8 @@ stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params
             }
         }
     }
-    collide_bgk<Q, FORCE>(f, d);
+    if (COLL == 0) collide_bgk<Q, FORCE>(f, d);
+    else collide_trt<Q, FORCE>(f, d);
     S *Bi = B + own;
 #pragma unroll
     for (int i = 0; i < Q; ++i) {                                        // a10

@@ -163,15 +163,10 @@ struct PullDirWall<Q, F, Q> {
                                                float (&)[Q]) {}
 };
 
-template <int COLL, int Q, bool FORCE>
-__device__ __forceinline__ void collide(float (&f)[Q], const Params &p) {
-    collide_bgk<Q, FORCE>(f, p);
-}
-
 constexpr int SC_THREADS = 256;
 
 // grid: x = tiles of BX*V cells along x, y = tiles of BY rows, z = plane.  blockDim = (BX, BY), BX*BY = SC_THREADS
-template <int Q, int F, int V, bool FORCE>
+template <int Q, int F, int V, bool FORCE, int COLL = 0>
 __global__ void __launch_bounds__(SC_THREADS)
 stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p) {
     typedef Elem<F> E;
@@ -206,7 +201,7 @@ stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F
         // ---- fast path: a3 load + decode, a5-a9 collide, a10 encode + store, all vectorised --------
         PullDir<Q, F, V, 0>::run(A, p.N, rows, x0, xm, xp, f);
 #pragma unroll
-        for (int j = 0; j < V; ++j) collide<0, Q, FORCE>(f[j], p);
+        for (int j = 0; j < V; ++j) collide<COLL, Q, FORCE>(f[j], p);
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             float o[V];
@@ -225,7 +220,7 @@ stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F
             const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
             float g[Q];
             PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, g);
-            collide<0, Q, FORCE>(g, p);
+            collide<COLL, Q, FORCE>(g, p);
 #pragma unroll
             for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + own + j, g[i]);
         }

@@ -20,7 +20,7 @@ namespace {
 constexpr int Q = LBM_Q, F = LBM_F;
 typedef typename Elem<F>::T T;
 
-template <int V, bool FORCE>
+template <int V, bool FORCE, int COLL = 0>
 cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) {
     const int tx = (p.nx + V - 1) / V;
     int bx = 1;
@@ -28,7 +28,7 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
     const int by = SC_THREADS / bx;
     const dim3 block(bx, by, 1);
     const dim3 grid((tx + bx - 1) / bx, (p.ny + by - 1) / by, p.nz);
-    stream_collide_kernel<Q, F, V, FORCE><<<grid, block, 0, st>>>((const T *)A, (T *)B, p);
+    stream_collide_kernel<Q, F, V, FORCE, COLL><<<grid, block, 0, st>>>((const T *)A, (T *)B, p);
     count_launch();
     return cudaGetLastError();
 }
@@ -56,10 +56,10 @@ BulkGeom bulk_geom(const Params &p, long long *tiles) {
     return g;
 }
 
-template <bool FORCE>
+template <bool FORCE, int COLL = 0>
 cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st) {
     typedef BulkShape<Q, F, BULK_NT> SH;
-    auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, FORCE>;
+    auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, FORCE, COLL>;
     static int ctas = 0;                      // resident CTAs on the device, resolved once per instantiation
     if (ctas == 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SH::SMEM);
@@ -86,7 +86,12 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
 }
 
 cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
-    (void)coll;
+    if (coll == 1) {
+        // TRT (R13): the staged kernel, or the per-thread kernel with one cell per thread whatever V asks for (the
+        // result does not depend on V)
+        if (V == VARIANT_BULK) return force ? launch_bulk<true, 1>(A, B, p, st) : launch_bulk<false, 1>(A, B, p, st);
+        return force ? launch_sc<1, true, 1>(A, B, p, st) : launch_sc<1, false, 1>(A, B, p, st);
+    }
     if (V == VARIANT_BULK) return force ? launch_bulk<true>(A, B, p, st) : launch_bulk<false>(A, B, p, st);
     switch (V * 2 + (force ? 1 : 0)) {
         case 2: return launch_sc<1, false>(A, B, p, st);
@@ -127,7 +132,13 @@ cudaError_t probe(const void *A, const Params &p, bool force, const long long *c
 }
 
 const char *name(int V, int coll, bool force) {
-    (void)coll;
+    if (coll == 1) {
+        if (V == VARIANT_BULK)
+            return force ? "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
+                         : "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0,COLL=TRT>";
+        return force ? "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=1,COLL=TRT>"
+                     : "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=0,COLL=TRT>";
+    }
     static const char *names[4][2] = {
         {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=0>",
          "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=1>"},

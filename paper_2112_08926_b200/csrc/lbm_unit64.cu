@@ -34,12 +34,13 @@ Params64 make64(const Params &p) {
     Params64 d;
     d.omega = 1.0 / (double)p.tau;
     d.one_m_omega = 1.0 - d.omega;
+    d.omega_minus = 1.0 / (0.5 + p.trt_lambda / ((double)p.tau - 0.5));   // R13
     d.F[0] = (double)p.fx; d.F[1] = (double)p.fy; d.F[2] = (double)p.fz;
     d.cs = 1.0 / std::sqrt(3.0);
     return d;
 }
 
-template <bool FORCE>
+template <bool FORCE, int COLL = 0>
 cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) {
     int bx = 32;
     while (bx < p.nx && bx < THREADS) bx <<= 1;
@@ -50,13 +51,14 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
     // registers) for double storage, where the kernel then runs at the HBM roofline; four (<= 64 registers, 28 bytes
     // of spills) for D2Q9 / D3Q19 float storage, which is bound by latency, not by bytes: 0.76 -> 0.83 of peak
     constexpr int MINB = (sizeof(S) == 4 && Q <= 19) ? 4 : 3;
-    stream_collide64_kernel<Q, S, FORCE, MINB><<<grid, block, 0, st>>>((const S *)A, (S *)B, p, make64(p));
+    stream_collide64_kernel<Q, S, FORCE, MINB, COLL><<<grid, block, 0, st>>>((const S *)A, (S *)B, p, make64(p));
     count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
-    (void)V; (void)coll;
+    (void)V;
+    if (coll == 1) return force ? launch_sc<true, 1>(A, B, p, st) : launch_sc<false, 1>(A, B, p, st);   // TRT (R13)
     return force ? launch_sc<true>(A, B, p, st) : launch_sc<false>(A, B, p, st);
 }
 
@@ -99,7 +101,10 @@ cudaError_t probe(const void *A, const Params &p, bool force, const long long *c
 }
 
 const char *name(int V, int coll, bool force) {
-    (void)V; (void)coll;
+    (void)V;
+    if (coll == 1)
+        return force ? "stream_collide64_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
+                     : "stream_collide64_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0,COLL=TRT>";
     return force ? "stream_collide64_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1>"
                  : "stream_collide64_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0>";
 }
