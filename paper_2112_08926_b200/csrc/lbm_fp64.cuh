@@ -143,13 +143,15 @@ __device__ __forceinline__ void collide_trt(double (&f)[Q], const Params64 &d) {
     double uF = 0.0;
     if (FORCE) uF = add(add(mul(u[0], d.F[0]), mul(u[1], d.F[1])), mul(u[2], d.F[2]));
     const double gp = sub(1.0, mul(0.5, d.omega)), gm = sub(1.0, mul(0.5, d.omega_minus));
+    const double hop = mul(0.5, d.omega), hom = mul(0.5, d.omega_minus);
     f[0] = fma_(d.one_m_omega, f[0], mul(d.omega, feq[0]));
     if (FORCE) f[0] = add(f[0], mul(mul(gp, wgt<Q>(0)), -mul(3.0, uF)));
 #pragma unroll
     for (int i = 1; i < Q; i += 2) {
-        const double fp = mul(0.5, add(f[i], f[i + 1])), fm = mul(0.5, sub(f[i], f[i + 1]));
-        const double ep = mul(0.5, add(feq[i], feq[i + 1])), em = mul(0.5, sub(feq[i], feq[i + 1]));
-        const double a = mul(d.omega, sub(fp, ep)), b = mul(d.omega_minus, sub(fm, em));
+        // the halves of f+-, e+- folded into the rates (exact scalings, as in lbm_lattice.cuh's TrtPairs)
+        const double dp = sub(add(f[i], f[i + 1]), add(feq[i], feq[i + 1]));
+        const double dm = sub(sub(f[i], f[i + 1]), sub(feq[i], feq[i + 1]));
+        const double a = mul(hop, dp), b = mul(hom, dm);
         double o1 = sub(sub(f[i], a), b), o2 = add(sub(f[i + 1], a), b);
         if (FORCE) {
             const double cu = cdot<Q>(i, u[0], u[1], u[2]);

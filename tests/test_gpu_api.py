@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 def test_create_rejects_bad_arguments():
     for kw, code in [(dict(nx=0), lbm.E_INVAL), (dict(velset=7), lbm.E_INVAL), (dict(tau=0.5), lbm.E_INVAL),
-                     (dict(ddf_format=9), lbm.E_INVAL), (dict(collision=lbm.TRT), lbm.E_UNSUPPORTED),
+                     (dict(ddf_format=9), lbm.E_INVAL), (dict(collision=2), lbm.E_INVAL),
                      (dict(velset=9, nz=2), lbm.E_INVAL)]:
         args = dict(nx=8, ny=8, nz=8, velset=19, ddf_format=0, tau=0.6, collision=0)
         args.update(kw)
