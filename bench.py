@@ -259,18 +259,20 @@ def run_ours(args):
         "gpu_launches": launches_total, "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(head, budget_s=args.cpu_seconds)
+        line["cpu_baseline"] = cpu_baseline(head, budget_s=args.cpu_seconds, collision=args.collision)
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
 
 
-def oracle_run(fmt_name, L, steps, warmup):
+def oracle_run(fmt_name, L, steps, warmup, collision="BGK"):
     """Time the CPU oracle, as it stands, on an L^3 sample of the workload.  Returns (mlups, cores, seconds)."""
     import oracle
     cores = oracle.set_threads(os.cpu_count() or 1)
     w = wl.perturbed_equilibrium(L, L, L, seed=SEED, tau=TAU)
     sim = oracle.from_workload(w, wl.FORMATS[fmt_name])
+    if collision == "TRT":
+        sim.set_collision(oracle.TRT)
     sim.step(warmup)
     t0 = time.perf_counter()
     sim.step(steps)
@@ -278,15 +280,15 @@ def oracle_run(fmt_name, L, steps, warmup):
     return L ** 3 * steps / dt / 1e6, cores, dt
 
 
-def cpu_baseline(fmt_name, budget_s=15.0):
+def cpu_baseline(fmt_name, budget_s=15.0, collision="BGK"):
     """The oracle on a BOUNDED sample: a 128^3 periodic box of the same recipe (beyond the LLC), step
     count sized from a 1-step probe so that the timed part takes about `budget_s` seconds."""
     L = 128
-    probe, cores, dt = oracle_run(fmt_name, L, 1, 1)
+    probe, cores, dt = oracle_run(fmt_name, L, 1, 1, collision)
     steps = max(2, min(200, int(budget_s / max(dt, 1e-3))))
-    mlups, cores, dt = oracle_run(fmt_name, L, steps, 0)
+    mlups, cores, dt = oracle_run(fmt_name, L, steps, 0, collision)
     return {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle",
-            "sample": f"D3Q19 BGK {fmt_name} storage, {L}^3 periodic box of the same recipe, {steps} steps, {dt:.1f} s"}
+            "sample": f"D3Q19 {collision} {fmt_name} storage, {L}^3 periodic box of the same recipe, {steps} steps, {dt:.1f} s"}
 
 
 def run_reference(args):
@@ -295,16 +297,16 @@ def run_reference(args):
         return
     K, W = args.steps, args.warmup
     L = 128
-    probe, cores, dt1 = oracle_run(HEADLINE, L, 1, 0)
+    probe, cores, dt1 = oracle_run(HEADLINE, L, 1, 0, args.collision)
     K_eff = max(1, min(K, int(120.0 / max(dt1, 1e-3))))       # keep the whole run within a few minutes
-    mlups, cores, dt = oracle_run(HEADLINE, L, K_eff, min(W, 2))
-    sample = (f"D3Q19 BGK {HEADLINE} storage, {L}^3 periodic sample box of the {args.size}^3 workload, "
+    mlups, cores, dt = oracle_run(HEADLINE, L, K_eff, min(W, 2), args.collision)
+    sample = (f"D3Q19 {args.collision} {HEADLINE} storage, {L}^3 periodic sample box of the {args.size}^3 workload, "
               f"{K_eff} timed steps, {dt:.1f} s, {cores} OpenMP threads")
     line = {"impl": "reference", "metric": METRIC, "value": round(mlups, 2), "unit": "MLUPs/s",
             "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": K_eff, "warmup": min(W, 2),
             "ms_per_step": round(dt / K_eff * 1e3, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"configs[4] bandwidth sweep: D3Q19 BGK periodic cube, perturbed equilibrium "
+            "config": {"workload": f"configs[4] bandwidth sweep: D3Q19 {args.collision} periodic cube, perturbed equilibrium "
                                    f"(seed {SEED}), tau {TAU}, storage format {HEADLINE}; CPU oracle on a bounded sample",
                        "sample": sample},
             "cpu_baseline": {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle", "sample": sample},
