@@ -118,6 +118,51 @@ def test_trt_equilibrium_boundary_cells(name):
     assert_parity(osim, gsim, name)
 
 
+# ---- the bench configuration (512^3 D3Q19 periodic, automatic kernel choice) with TRT ------------------------------
+# As tests/test_gpu_lbm.py's full-size test: after n steps a cell depends only on the initial fields within n cells of
+# it, so sampled 14^3 blocks (some across the periodic faces) are stepped by the oracle as boxes of their own and
+# their 8^3 cores must agree with the GPU bit for bit.
+FULL_L, FULL_STEPS, BLK = 512, 3, 14
+
+
+@pytest.fixture(scope="module")
+def full_size_workload():
+    return wl.perturbed_equilibrium(FULL_L, FULL_L, FULL_L, seed=20211208, tau=0.6)
+
+
+def _block(field, origin, L):
+    ix = [np.arange(o, o + BLK) % L for o in origin]
+    return field[..., ix[2][:, None, None], ix[1][None, :, None], ix[0][None, None, :]]
+
+
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "P16_0S"])
+def test_trt_full_size_sampled_blocks(full_size_workload, name):
+    w, L = full_size_workload, FULL_L
+    g = lbm.from_workload(w, name, collision=lbm.TRT)
+    assert "COLL=TRT" in g.kernel_name and ("bulk" in g.kernel_name) == (name != "FP32")
+    g.step(FULL_STEPS)
+    grho, gu = g.read_rho_u()
+    g.close()
+    assert np.all(np.isfinite(grho))
+    grho, gu = grho.reshape(L, L, L), gu.reshape(3, L, L, L)
+    rho0, u0 = w.rho.reshape(L, L, L), w.u.reshape(3, L, L, L)
+    rng = np.random.default_rng(7)
+    origins = [(-7, -7, -7), (L - 7, 100, 200), (300, L - 7, 17), (40, 50, L - 7), (0, 0, 0)]
+    origins += [tuple(int(v) for v in rng.integers(0, L, 3)) for _ in range(5)]
+    c = slice(3, BLK - 3)
+    for o in origins:
+        sub = wl.Workload("block", BLK, BLK, BLK, 19, w.tau, np.ascontiguousarray(_block(rho0, o, L)).reshape(-1),
+                          np.ascontiguousarray(_block(u0, o, L)).reshape(3, -1), np.zeros(BLK ** 3, np.uint8))
+        osim = oracle.from_workload(sub, FORMATS[name])
+        osim.set_collision(oracle.TRT)
+        osim.step(FULL_STEPS)
+        orho, ou = osim.read_rho_u()
+        orho = orho.reshape(BLK, BLK, BLK)[c, c, c]
+        ou = ou.reshape(3, BLK, BLK, BLK)[:, c, c, c]
+        assert np.array_equal(_block(grho, o, L)[c, c, c].view(np.uint32), orho.view(np.uint32)), (name, o)
+        assert np.array_equal(_block(gu, o, L)[:, c, c, c].view(np.uint32), ou.view(np.uint32)), (name, o)
+
+
 # ---- what the method fixes, on the product alone -----------------------------------------------------------
 def test_trt_with_equal_rates_matches_bgk_to_rounding():
     """Lambda = (tau - 1/2)^2 makes omega- = omega+ (R13): the TRT run then follows the BGK run up to rounding."""
