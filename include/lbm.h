@@ -90,7 +90,6 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream);
  *   1, 2, 4            the per-thread kernel with that many cells per thread along x (nx a multiple of it);
  *   LBM_VARIANT_BULK   the shared-memory-staged kernel: DDF rows move by cp.async.bulk, persistent CTAs
  *                      (nx a multiple of 16).
- * LBM_TRT handles run 4 cells per thread as 2.
  * lbm_set_cells_per_thread(h, v) = lbm_set_variant(h, v) restricted to v in {0, 1, 2, 4}. */
 enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16 };
 int lbm_set_variant(lbm_t *h, int variant);

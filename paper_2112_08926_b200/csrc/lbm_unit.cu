@@ -87,9 +87,9 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
 
 cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
     if (coll == 1) {
-        // TRT (R13): the staged kernel, or the per-thread kernel with one or two cells per thread (four run as two: the
-        // result does not depend on V)
+        // TRT (R13): the staged kernel, or the per-thread kernel with one, two or four cells per thread
         if (V == VARIANT_BULK) return force ? launch_bulk<true, 1>(A, B, p, st) : launch_bulk<false, 1>(A, B, p, st);
+        if (V == 4 && p.nx % 4 == 0) return force ? launch_sc<4, true, 1>(A, B, p, st) : launch_sc<4, false, 1>(A, B, p, st);
         if (V >= 2 && p.nx % 2 == 0) return force ? launch_sc<2, true, 1>(A, B, p, st) : launch_sc<2, false, 1>(A, B, p, st);
         return force ? launch_sc<1, true, 1>(A, B, p, st) : launch_sc<1, false, 1>(A, B, p, st);
     }
@@ -137,6 +137,9 @@ const char *name(int V, int coll, bool force) {
         if (V == VARIANT_BULK)
             return force ? "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
                          : "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0,COLL=TRT>";
+        if (V == 4)
+            return force ? "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=1,COLL=TRT>"
+                         : "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=0,COLL=TRT>";
         if (V >= 2)
             return force ? "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=1,COLL=TRT>"
                          : "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=0,COLL=TRT>";

@@ -25,13 +25,13 @@ TOL = {name: (1e-6 if name == "FP32" else 1e-3) for name in ALL_FORMATS}
 F64_FORMATS = {"FP64": (oracle.FP64, np.uint64), "FP64_FP32": (oracle.FP32, np.uint32)}
 
 
-def run_pair(w, name, steps, lam=None, variant=0):
+def run_pair(w, name, steps, lam=None, variant=0, cells_per_thread=0):
     if name in F64_FORMATS:
         w = dataclasses.replace(w, tau=float(np.float32(w.tau)), force=tuple(float(np.float32(v)) for v in w.force))
         osim = oracle.from_workload(w, F64_FORMATS[name][0], oracle.ARITH_F64)
     else:
         osim = oracle.from_workload(w, FORMATS[name])
-    gsim = lbm.from_workload(w, name, collision=lbm.TRT, variant=variant)
+    gsim = lbm.from_workload(w, name, collision=lbm.TRT, variant=variant, cells_per_thread=cells_per_thread)
     if lam is None:
         osim.set_collision(oracle.TRT)
     else:
@@ -79,6 +79,18 @@ def test_trt_walls_moving_walls_force(q, shape, name, lam):
         w = wl.random_walls(w, 0.12, seed=43, moving_fraction=0.5)
     w.force = (1e-5, -2e-5, 0.0 if q == 9 else 3e-5)
     osim, gsim = run_pair(w, name, 20, lam=lam)
+    assert_parity(osim, gsim, name)
+
+
+@pytest.mark.parametrize("q,shape", [(19, (24, 9, 7)), (9, (40, 17, 1))])
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "P16_2C"])
+@pytest.mark.parametrize("v", [1, 2, 4])
+def test_trt_cells_per_thread_variants(q, shape, name, v):
+    w = wl.perturbed_equilibrium(*shape, seed=67, velset=q, tau=0.7)
+    w = wl.random_walls(w, 0.1, seed=71, moving_fraction=0.5)
+    w.force = (1e-5, -2e-5, 0.0 if q == 9 else 3e-5)
+    osim, gsim = run_pair(w, name, 15, cells_per_thread=v)
+    assert f"V={v}," in gsim.kernel_name
     assert_parity(osim, gsim, name)
 
 
