@@ -89,9 +89,11 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream);
  *   LBM_VARIANT_AUTO   the library chooses;
  *   1, 2, 4            the per-thread kernel with that many cells per thread along x (nx a multiple of it);
  *   LBM_VARIANT_BULK   the shared-memory-staged kernel: DDF rows move by cp.async.bulk, persistent CTAs
- *                      (nx a multiple of 16).
+ *                      (nx a multiple of 16);
+ *   LBM_VARIANT_STAGED the warp-specialised staged kernel: one producer warp per CTA moves loads AND stores with
+ *                      cp.async.bulk, the other warps only compute (nx a multiple of 16).
  * lbm_set_cells_per_thread(h, v) = lbm_set_variant(h, v) restricted to v in {0, 1, 2, 4}. */
-enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16 };
+enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16, LBM_VARIANT_STAGED = 32 };
 int lbm_set_variant(lbm_t *h, int variant);
 int lbm_set_cells_per_thread(lbm_t *h, int v);
 
@@ -114,8 +116,11 @@ int lbm_init_device(lbm_t *h, const float *rho_dev, const float *u_dev);
 
 /* Advance n >= 0 time steps: n launches of the fused stream-collide kernel (Listing 2,
  * PAPER.md:1014-1042; eqs (24)-(28)), alternating the two buffers.
- * Asynchronous on the handle's stream. */
+ * Asynchronous on the handle's stream.  On boxes of up to 2^23 cells, where a launch costs as much as the kernel, runs of
+ * 32 launches are captured into a CUDA graph once and replayed (same kernels, same arguments, same results);
+ * lbm_set_graphs(h, 0) turns that off (for before / after measurements), lbm_set_graphs(h, 1) on again (default). */
 int lbm_step(lbm_t *h, int n);
+int lbm_set_graphs(lbm_t *h, int enable);
 
 /* Density and velocity "after the steps done so far" = local moments of the current buffer (R12;
  * PAPER.md:428, 951-968); wall cells return the values given to lbm_init.  Either pointer may be NULL.
@@ -159,6 +164,11 @@ int lbm_codec_decode_device(int ddf_format, const unsigned short *codes_dev, flo
  * through the pair decoders and all 2^32 FP32 bit patterns through the pair encoder, compared bit for bit (NaN
  * inputs excepted).  *mismatches (HOST) receives the number of differences (0 = identical).  Synchronous. */
 int lbm_codec_pair_selftest(int ddf_format, long long *mismatches);
+
+/* Device self-check of the staged kernel's velocity division (u = j / rho with one shared reciprocal, lbm_lattice.cuh
+ * div3) against the IEEE division it replaces: about 10^8 (numerator, denominator) pairs incl. zero numerators of both
+ * signs, compared bit for bit.  *mismatches (HOST) receives the number of differences (0 = identical).  Synchronous. */
+int lbm_div_selftest(long long *mismatches);
 
 /* ---- sizes -------------------------------------------------------------------------------------*/
 /* bytes of ONE DDF buffer: q * N * sizeof(element), rounded up to a multiple of 256 */

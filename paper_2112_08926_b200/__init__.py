@@ -29,7 +29,7 @@ FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C"
            "FP64": 7, "FP64_FP32": 8}     # 7, 8: FP64 arithmetic with double / float storage
 FORMAT_NAMES = {v: k for k, v in FORMATS.items()}
 FLAG_WALL, FLAG_EQ = 0x01, 0x02
-VARIANT_AUTO, VARIANT_BULK = 0, 16
+VARIANT_AUTO, VARIANT_BULK, VARIANT_STAGED = 0, 16, 32
 OK, E_INVAL, E_UNSUPPORTED, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/lbm.h declares: (restype, argtypes)
@@ -44,6 +44,7 @@ SYMBOLS = {
     "lbm_init": (_i, [_p, _p, _p]),
     "lbm_init_device": (_i, [_p, _p, _p]),
     "lbm_step": (_i, [_p, _i]),
+    "lbm_set_graphs": (_i, [_p, _i]),
     "lbm_read_rho_u": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_device": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_f64": (_i, [_p, _p, _p]),
@@ -58,6 +59,7 @@ SYMBOLS = {
     "lbm_codec_encode_device": (_i, [_i, _p, _p, _ll, _p]),
     "lbm_codec_decode_device": (_i, [_i, _p, _p, _ll, _p]),
     "lbm_codec_pair_selftest": (_i, [_i, C.POINTER(_ll)]),
+    "lbm_div_selftest": (_i, [C.POINTER(_ll)]),
     "lbm_ddf_buffer_bytes": (_ll, [_i, _i, _i, _i, _i]),
     "lbm_bytes_per_cell": (_ll, [_i, _i]),
     "lbm_kernel_name": (C.c_char_p, [_p]),
@@ -207,6 +209,9 @@ class Simulation:
     def step(self, n: int = 1):
         _check(lib().lbm_step(self._h, int(n)))
 
+    def set_graphs(self, enable: bool):
+        _check(lib().lbm_set_graphs(self._h, 1 if enable else 0))
+
     def sync(self):
         _check(lib().lbm_sync(self._h))
 
@@ -218,6 +223,10 @@ class Simulation:
             u = np.empty((3, self.N), np.float32)
         else:
             rho, u = out
+            for a, n in ((rho, self.N), (u, 3 * self.N)):
+                if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous and a.size == n
+                        and a.flags.writeable):
+                    raise ValueError("read_rho_u(out=(rho, u)): writable C-contiguous float32 arrays of N and 3N entries")
         _check(lib().lbm_read_rho_u(self._h, _np_ptr(rho), _np_ptr(u)))
         return rho, u
 
@@ -287,4 +296,11 @@ def codec_pair_selftest(ddf_format) -> int:
     exhaustive over all codes / all FP32 patterns, computed on the GPU (0 = identical)."""
     n = _ll(0)
     _check(lib().lbm_codec_pair_selftest(_fmt(ddf_format), C.byref(n)))
+    return int(n.value)
+
+
+def div_selftest() -> int:
+    """Number of bit mismatches between the staged kernel's shared-reciprocal division and IEEE division (0 = identical)."""
+    n = _ll(0)
+    _check(lib().lbm_div_selftest(C.byref(n)))
     return int(n.value)

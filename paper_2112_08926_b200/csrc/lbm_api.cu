@@ -33,6 +33,12 @@ struct lbm {
     int cur;                   // index of the buffer holding the current state
     float *rho0, *u0;          // device copies of the init fields, kept only when the box has walls
     unsigned *bounce;          // device, N words: which directions bounce (lbm_lattice.cuh), only when the box has walls
+    unsigned *fix_off;         // device: per-tile lists of flagged cell pairs for the staged kernel (lbm_stage.cuh), built on
+    uint2 *fix_cells; // first use after lbm_set_flags, only when the box has flagged cells
+    cudaGraphExec_t gexec[2];  // lbm_step on small boxes: GRAPH_STEPS launches captured once, starting from buffer 0 / 1
+    bool graphs;               // lbm_set_graphs
+    void *scratch;             // device staging area of the host-pointer calls (lbm_init, lbm_read_rho_u*), kept between calls
+    size_t scratch_bytes;
     long long steps;
     bool inited;
     int V;                     // stream_collide variant in use: 1, 2, 4 cells per thread or LBM_VARIANT_BULK
@@ -80,12 +86,35 @@ Params make_params(const lbm *h) {
     p.u0 = h->u0;
     p.bounce = h->bounce;
     p.tau = h->tau;
+    p.fix_off = h->fix_off;
+    p.fix_cells = h->fix_cells;
     return p;
 }
 
 int enter(lbm *h) {
     if (!h) return fail(LBM_E_INVAL, "null handle");
     LBM_CUDA_TRY(cudaSetDevice(h->device));
+    return LBM_OK;
+}
+
+// One staging buffer per handle for the calls that take host pointers: allocated at the first such call, grown when a
+// later call needs more, freed by lbm_destroy (a cudaMalloc / cudaFree pair of gigabytes per call costs milliseconds
+// and synchronises the device).
+// Small boxes are launch-bound (BASELINE configs 1 and 2: 32 768 and 16 384 cells, a kernel of a few microseconds): lbm_step
+// captures GRAPH_STEPS consecutive launches (an even number: the A/B buffers end where they started) into a CUDA graph
+// once and replays it.  Anything that changes a kernel argument drops the graphs.
+constexpr int GRAPH_STEPS = 32;
+constexpr long long GRAPH_MAX_CELLS = 1LL << 23;
+void drop_graphs(lbm *h) {
+    for (int b = 0; b < 2; ++b)
+        if (h->gexec[b]) { cudaGraphExecDestroy(h->gexec[b]); h->gexec[b] = nullptr; }
+}
+
+int ensure_scratch(lbm *h, size_t bytes) {
+    if (h->scratch_bytes >= bytes) return LBM_OK;
+    if (h->scratch) { cudaFree(h->scratch); h->scratch = nullptr; h->scratch_bytes = 0; }
+    LBM_CUDA_TRY(cudaMalloc(&h->scratch, bytes));
+    h->scratch_bytes = bytes;
     return LBM_OK;
 }
 
@@ -105,24 +134,22 @@ int ensure_ddf(lbm *h) {
     return LBM_OK;
 }
 
-// Kernel variant.  Automatic choice, from the bandwidth sweep recorded in DESIGN.md section 6:
-//   * FP32 storage, no flagged cells: the per-thread kernel (it runs at the HBM roofline);
-//   * 16-bit formats, D3Q19 / D3Q27, rows 16-cell aligned and >= 64 cells, box >= 2^20 cells: the
-//     shared-memory-staged kernel (lbm_bulk.cuh), which lifts them out of the issue bound;
-//   * D2Q9 (9 streams: the staged kernel's per-tile bookkeeping does not pay) and small boxes (L2-resident,
-//     launch-bound): the per-thread kernel, 4 cells per thread for D2Q9, else 2.
+// Kernel variant.  Automatic choice, from the sweeps recorded in DESIGN.md section 6:
+//   * FP64 arithmetic: one kernel, one cell per thread (lbm_fp64.cuh);
+//   * rows 16-cell aligned and >= 64 cells, box >= 2^20 cells, and either a 16-bit format or a box with flagged cells:
+//     the warp-specialised staged kernel (lbm_stage.cuh) -- it lifts the 16-bit formats out of the issue bound and
+//     handles flagged cells in a compacted list pass instead of a divergent slow path;
+//   * FP32 storage without flagged cells: the per-thread kernel, which runs at the HBM roofline;
+//   * everything else (ragged rows, small L2-resident / launch-bound boxes): the per-thread kernel, 4 cells per thread
+//     for D2Q9 16-bit, else 2.
 int pick_variant(const lbm *h) {
-    if (arith64(h->fmt)) return 1;            // FP64 arithmetic: one kernel, one cell per thread (lbm_fp64.cuh)
+    if (arith64(h->fmt)) return 1;
     int want = h->V_request;
-    if (want == 0) {
-        const char *env = getenv("LBM_VARIANT");
-        if (env && *env) want = atoi(env);
-    }
+    const bool staged_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->staged_tile_cells() - 1) / h->ops->staged_tile_cells()) * h->ny * h->nz < 0x7FFFFFFFLL;
+    if (want == LBM_VARIANT_STAGED && staged_ok) return LBM_VARIANT_STAGED;
     const bool bulk_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->bulk_tile_cells() - 1) / h->ops->bulk_tile_cells()) * h->ny * h->nz <= 0x7FFFFFFFLL;
     if (want == LBM_VARIANT_BULK && bulk_ok) return LBM_VARIANT_BULK;
-    // (FP32 storage in a box with flagged cells also gains: the staged kernel's near-wall path has no serial gathers)
-    if (want == 0 && bulk_ok && (h->fmt != LBM_FP32 || h->has_walls) && h->q != LBM_D2Q9 && h->nx >= 64 && h->N >= (1LL << 20))
-        return LBM_VARIANT_BULK;
+    if (want == 0 && staged_ok && (h->fmt != LBM_FP32 || h->has_walls) && h->nx >= 64 && h->N >= (1LL << 20)) return LBM_VARIANT_STAGED;
     if (want != 1 && want != 2 && want != 4) want = (h->q == LBM_D2Q9 && h->fmt != LBM_FP32) ? 4 : 2;
     while (want > 1 && h->nx % want != 0) want >>= 1;
     return want;
@@ -171,6 +198,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, i
     h->tau = tau;
     h->omega = 1.0f / tau;
     h->trt_lambda = 3.0 / 16.0;
+    h->graphs = true;
     for (int a = 0; a < 3; ++a) {
         h->force[a] = force ? force[a] : 0.0f;
         if (h->force[a] != 0.0f) h->has_force = true;
@@ -196,11 +224,14 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream) {
     if ((ddf_a == nullptr) != (ddf_b == nullptr)) return fail(LBM_E_INVAL, "lbm_bind: bind both DDF buffers or neither");
     if (ddf_a) {
         if (((size_t)ddf_a | (size_t)ddf_b) & 15) return fail(LBM_E_INVAL, "lbm_bind: DDF buffers must be 16-byte aligned");
-        if (ddf_a == ddf_b) return fail(LBM_E_INVAL, "lbm_bind: the two DDF buffers must be distinct");
+        const long long need = lbm_ddf_buffer_bytes(h->nx, h->ny, h->nz, h->q, h->fmt);
+        const char *pa = (const char *)ddf_a, *pb = (const char *)ddf_b;
+        if ((pa <= pb ? pb - pa : pa - pb) < need) return fail(LBM_E_INVAL, "lbm_bind: the two DDF buffers overlap");
         if (h->owns_ddf) { cudaFree(h->ddf[0]); cudaFree(h->ddf[1]); h->owns_ddf = false; }
         h->ddf[0] = ddf_a;
         h->ddf[1] = ddf_b;
     }
+    drop_graphs(h);
     h->stream = (cudaStream_t)cuda_stream;
     h->bound = true;
     return LBM_OK;
@@ -208,14 +239,16 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream) {
 
 int lbm_set_variant(lbm_t *h, int v) {
     if (int rc = enter(h)) return rc;
-    if (v != LBM_VARIANT_AUTO && v != 1 && v != 2 && v != 4 && v != LBM_VARIANT_BULK)
-        return fail(LBM_E_INVAL, "lbm_set_variant: 0 (auto), 1, 2, 4 (cells per thread) or LBM_VARIANT_BULK");
+    if (v != LBM_VARIANT_AUTO && v != 1 && v != 2 && v != 4 && v != LBM_VARIANT_BULK && v != LBM_VARIANT_STAGED)
+        return fail(LBM_E_INVAL, "lbm_set_variant: 0 (auto), 1, 2, 4 (cells per thread), LBM_VARIANT_BULK or LBM_VARIANT_STAGED");
     if ((v == 2 || v == 4) && h->nx % v != 0) return fail(LBM_E_INVAL, "lbm_set_variant: nx must be a multiple of the cells per thread");
-    if (v == LBM_VARIANT_BULK && h->nx % 16 != 0) return fail(LBM_E_INVAL, "lbm_set_variant: the staged kernel needs nx to be a multiple of 16");
-    if (v == LBM_VARIANT_BULK && arith64(h->fmt)) return fail(LBM_E_UNSUPPORTED, "lbm_set_variant: the FP64-arithmetic formats have no staged kernel");
+    const bool staged = v == LBM_VARIANT_BULK || v == LBM_VARIANT_STAGED;
+    if (staged && h->nx % 16 != 0) return fail(LBM_E_INVAL, "lbm_set_variant: the staged kernels need nx to be a multiple of 16");
+    if (staged && arith64(h->fmt)) return fail(LBM_E_UNSUPPORTED, "lbm_set_variant: the FP64-arithmetic formats have no staged kernel");
+    drop_graphs(h);
     h->V_request = v;
     h->V = pick_variant(h);
-    if (v == LBM_VARIANT_BULK && h->V != v) return fail(LBM_E_INVAL, "lbm_set_variant: box too large for the staged kernel's tile index");
+    if (staged && h->V != v) return fail(LBM_E_INVAL, "lbm_set_variant: box too large for the staged kernel's tile index");
     return LBM_OK;
 }
 
@@ -224,6 +257,7 @@ int lbm_set_trt_lambda(lbm_t *h, double lambda) {
     if (h->collision != LBM_TRT) return fail(LBM_E_STATE, "lbm_set_trt_lambda: the handle was not created with LBM_TRT");
     if (!(lambda > 0.0) || !(lambda < 1e30)) return fail(LBM_E_INVAL, "lbm_set_trt_lambda: Lambda must be positive and finite");
     // FP32 arithmetic sees the FP32 value of Lambda, FP64 arithmetic the double as given
+    drop_graphs(h);
     h->trt_lambda = arith64(h->fmt) ? lambda : (double)(float)lambda;
     return LBM_OK;
 }
@@ -244,6 +278,9 @@ int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
         walls |= flags[n] != 0;
     }
     h->has_walls = walls;
+    drop_graphs(h);
+    if (h->fix_off) { cudaFree(h->fix_off); h->fix_off = nullptr; }       // the lists belong to the old flags
+    if (h->fix_cells) { cudaFree(h->fix_cells); h->fix_cells = nullptr; }
     if (!walls) {
         LBM_CUDA_TRY(cudaMemsetAsync(h->flags, 0, (size_t)h->N, h->stream));
         LBM_CUDA_TRY(cudaStreamSynchronize(h->stream));
@@ -262,6 +299,9 @@ int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
 
 static int init_from_device(lbm *h, const float *rho_dev, const float *u_dev) {
     if (int rc = ensure_ddf(h)) return rc;
+    drop_graphs(h);
+    if (h->fix_off) { cudaFree(h->fix_off); h->fix_off = nullptr; }       // the lists carry the "wall moves" bits of the old fields
+    if (h->fix_cells) { cudaFree(h->fix_cells); h->fix_cells = nullptr; }
     const float *r = rho_dev, *u = u_dev;
     if (h->has_walls) {                          // wall velocity (R9) and wall read-out (R12) need the init fields later
         if (!h->rho0) LBM_CUDA_TRY(cudaMalloc((void **)&h->rho0, (size_t)h->N * 4));
@@ -296,19 +336,27 @@ int lbm_init(lbm_t *h, const float *rho, const float *u) {
         r = h->rho0;
         v = h->u0;
     } else {
-        LBM_CUDA_TRY(cudaMalloc((void **)&r, (size_t)h->N * 4));
-        cudaError_t e = cudaMalloc((void **)&v, (size_t)h->N * 12);
-        if (e != cudaSuccess) { cudaFree(r); LBM_CUDA_TRY(e); }
+        if (int rc = ensure_scratch(h, (size_t)h->N * 16)) return rc;
+        r = (float *)h->scratch;
+        v = r + h->N;
     }
     cudaError_t e = cudaMemcpyAsync(r, rho, (size_t)h->N * 4, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(v, u, (size_t)h->N * 12, cudaMemcpyHostToDevice, h->stream);
     int rc = LBM_OK;
     if (e == cudaSuccess) rc = init_from_device(h, r, v);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
-    if (!h->has_walls) { cudaFree(r); cudaFree(v); }
     LBM_CUDA_TRY(e);
     if (rc) return rc;
     LBM_CUDA_TRY(e2);
+    return LBM_OK;
+}
+
+static int step_plain(lbm *h, const Params &p, int n) {
+    for (int k = 0; k < n; ++k) {
+        LBM_CUDA_TRY(h->ops->stream_collide(h->ddf[h->cur], h->ddf[1 - h->cur], p, h->V, h->collision, h->has_force, h->stream));
+        h->cur = 1 - h->cur;
+        h->steps += 1;
+    }
     return LBM_OK;
 }
 
@@ -316,12 +364,50 @@ int lbm_step(lbm_t *h, int n) {
     if (int rc = enter(h)) return rc;
     if (n < 0) return fail(LBM_E_INVAL, "lbm_step: n must be >= 0");
     if (!h->inited) return fail(LBM_E_STATE, "lbm_step: call lbm_init first");
+    if (h->V == LBM_VARIANT_STAGED && h->has_walls && !h->fix_off && n > 0)
+        LBM_CUDA_TRY(h->ops->build_fix_lists(make_params(h), &h->fix_off, &h->fix_cells, h->stream));
     const Params p = make_params(h);
-    for (int k = 0; k < n; ++k) {
-        LBM_CUDA_TRY(h->ops->stream_collide(h->ddf[h->cur], h->ddf[1 - h->cur], p, h->V, h->collision, h->has_force, h->stream));
-        h->cur = 1 - h->cur;
-        h->steps += 1;
+    if (h->graphs && h->N <= GRAPH_MAX_CELLS && n >= 2 + GRAPH_STEPS) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(h->stream, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusNone) {
+            if (!h->gexec[h->cur]) {
+                // both directions once outside the capture (first launches set function attributes, build tables)
+                if (int rc = step_plain(h, p, 2)) return rc;
+                n -= 2;
+                cudaGraph_t graph = nullptr;
+                const long long steps0 = h->steps;
+                const int cur0 = h->cur;
+                cudaError_t e = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal);
+                int rc = LBM_OK;
+                if (e == cudaSuccess) {
+                    rc = step_plain(h, p, GRAPH_STEPS);
+                    e = cudaStreamEndCapture(h->stream, &graph);
+                }
+                h->steps = steps0;                              // captured, not executed
+                h->cur = cur0;
+                lbmk::count_launch(-(long long)GRAPH_STEPS);
+                if (rc == LBM_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&h->gexec[cur0], graph, 0);
+                if (graph) cudaGraphDestroy(graph);
+                if (rc != LBM_OK || e != cudaSuccess) {          // no graph: plain launches below
+                    (void)cudaGetLastError();
+                    h->gexec[cur0] = nullptr;
+                }
+            }
+            while (h->gexec[h->cur] && n >= GRAPH_STEPS) {
+                LBM_CUDA_TRY(cudaGraphLaunch(h->gexec[h->cur], h->stream));
+                lbmk::count_launch(GRAPH_STEPS);
+                h->steps += GRAPH_STEPS;
+                n -= GRAPH_STEPS;
+            }
+        }
     }
+    return step_plain(h, p, n);
+}
+
+int lbm_set_graphs(lbm_t *h, int enable) {
+    if (int rc = enter(h)) return rc;
+    h->graphs = enable != 0;
+    if (!h->graphs) drop_graphs(h);
     return LBM_OK;
 }
 
@@ -337,13 +423,12 @@ int lbm_read_rho_u(lbm_t *h, float *rho, float *u) {
     if (int rc = enter(h)) return rc;
     if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u: call lbm_init first");
     if (!rho && !u) return LBM_OK;
-    float *d = nullptr;
-    LBM_CUDA_TRY(cudaMalloc((void **)&d, (size_t)h->N * 16));
+    if (int rc = ensure_scratch(h, (size_t)h->N * 16)) return rc;
+    float *d = (float *)h->scratch;
     cudaError_t e = h->ops->read(h->ddf[h->cur], make_params(h), h->has_force, rho ? d : nullptr, u ? d + h->N : nullptr, h->stream);
     if (e == cudaSuccess && rho) e = cudaMemcpyAsync(rho, d, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && u) e = cudaMemcpyAsync(u, d + h->N, (size_t)h->N * 12, cudaMemcpyDeviceToHost, h->stream);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
-    cudaFree(d);
     LBM_CUDA_TRY(e);
     LBM_CUDA_TRY(e2);
     return LBM_OK;
@@ -354,13 +439,12 @@ int lbm_read_rho_u_f64(lbm_t *h, double *rho, double *u) {
     if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u_f64: call lbm_init first");
     if (!h->ops->read64) return fail(LBM_E_UNSUPPORTED, "lbm_read_rho_u_f64: FP64-arithmetic formats only (LBM_FP64, LBM_FP64_FP32)");
     if (!rho && !u) return LBM_OK;
-    double *d = nullptr;
-    LBM_CUDA_TRY(cudaMalloc((void **)&d, (size_t)h->N * 32));
+    if (int rc = ensure_scratch(h, (size_t)h->N * 32)) return rc;
+    double *d = (double *)h->scratch;
     cudaError_t e = h->ops->read64(h->ddf[h->cur], make_params(h), h->has_force, rho ? d : nullptr, u ? d + h->N : nullptr, h->stream);
     if (e == cudaSuccess && rho) e = cudaMemcpyAsync(rho, d, (size_t)h->N * 8, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess && u) e = cudaMemcpyAsync(u, d + h->N, (size_t)h->N * 24, cudaMemcpyDeviceToHost, h->stream);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
-    cudaFree(d);
     LBM_CUDA_TRY(e);
     LBM_CUDA_TRY(e2);
     return LBM_OK;
@@ -373,16 +457,15 @@ int lbm_read_rho_u_at(lbm_t *h, const long long *cells, int count, float *rho, f
     if (count == 0) return LBM_OK;
     for (int k = 0; k < count; ++k)
         if (cells[k] < 0 || cells[k] >= h->N) return fail(LBM_E_INVAL, "lbm_read_rho_u_at: cell index out of range");
-    char *d = nullptr;
     const size_t cb = (size_t)count * 8, fb = (size_t)count * 16;
-    LBM_CUDA_TRY(cudaMalloc((void **)&d, cb + fb));
+    if (int rc = ensure_scratch(h, cb + fb)) return rc;
+    char *d = (char *)h->scratch;
     float *df = (float *)(d + cb);
     cudaError_t e = cudaMemcpyAsync(d, cells, cb, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) e = h->ops->probe(h->ddf[h->cur], make_params(h), h->has_force, (const long long *)d, count, df, df + count, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(rho, df, (size_t)count * 4, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(u, df + count, (size_t)count * 12, cudaMemcpyDeviceToHost, h->stream);
     cudaError_t e2 = cudaStreamSynchronize(h->stream);
-    cudaFree(d);
     LBM_CUDA_TRY(e);
     LBM_CUDA_TRY(e2);
     return LBM_OK;
@@ -416,11 +499,15 @@ int lbm_destroy(lbm_t *h) {
     if (!h) return LBM_OK;
     cudaSetDevice(h->device);
     cudaStreamSynchronize(h->stream);
+    drop_graphs(h);
     if (h->owns_ddf) { cudaFree(h->ddf[0]); cudaFree(h->ddf[1]); }
     if (h->flags) cudaFree(h->flags);
     if (h->rho0) cudaFree(h->rho0);
     if (h->u0) cudaFree(h->u0);
     if (h->bounce) cudaFree(h->bounce);
+    if (h->fix_off) cudaFree(h->fix_off);
+    if (h->fix_cells) cudaFree(h->fix_cells);
+    if (h->scratch) cudaFree(h->scratch);
     (void)cudaGetLastError();
     delete h;
     return LBM_OK;
@@ -473,6 +560,19 @@ int lbm_codec_pair_selftest(int ddf_format, long long *mismatches) {
     LBM_CUDA_TRY(cudaMalloc((void **)&d, 8));
     cudaError_t e = cudaMemset(d, 0, 8);
     if (e == cudaSuccess) e = lbmk::launch_pair_selftest(ddf_format, d, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(&hval, d, 8, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    LBM_CUDA_TRY(e);
+    *mismatches = (long long)hval;
+    return LBM_OK;
+}
+
+int lbm_div_selftest(long long *mismatches) {
+    if (!mismatches) return fail(LBM_E_INVAL, "lbm_div_selftest: mismatches is NULL");
+    unsigned long long *d = nullptr, hval = 0;
+    LBM_CUDA_TRY(cudaMalloc((void **)&d, 8));
+    cudaError_t e = cudaMemset(d, 0, 8);
+    if (e == cudaSuccess) e = lbmk::launch_div_selftest(d, 0);
     if (e == cudaSuccess) e = cudaMemcpy(&hval, d, 8, cudaMemcpyDeviceToHost);
     cudaFree(d);
     LBM_CUDA_TRY(e);

@@ -2,9 +2,11 @@
 // stand-alone codec kernels behind lbm_codec_encode / lbm_codec_decode (bit-level parity tests).
 #include <atomic>
 #include <cstdio>
+#include <mutex>
 
 #include "lbm_internal.h"
 #include "lbm_kernels.cuh"
+#include "lbm_bulk.cuh"
 
 namespace lbmk {
 
@@ -90,6 +92,121 @@ cudaError_t launch_mark_moving(int q, unsigned *bounce, const float *u0, int nx,
     return cudaGetLastError();
 }
 
+// ---- per-tile lists of flagged cells (built at the first step after lbm_set_flags / lbm_init, for the staged kernel's
+// tile geometry; lbm_stage.cuh) ---------------------------------------------------------------------------
+// counts[t] = number of cells of tile t with a flag bit set (wall, equilibrium boundary, next to a wall)
+__global__ void __launch_bounds__(128) fix_count_kernel(const Params p, const BulkGeom g, unsigned *__restrict__ counts) {
+    __shared__ unsigned total;
+    for (int t = blockIdx.x; t < g.n_tiles; t += gridDim.x) {
+        if (threadIdx.x == 0) total = 0;
+        __syncthreads();
+        const TileCoord c = tile_coord(t, g, p);
+        const int cells = c.rows * c.w;
+        const long long first = (long long)p.nx * (c.y + (long long)p.ny * c.z) + c.x0;
+        unsigned n = 0;
+        for (int ci = threadIdx.x; ci < cells; ci += blockDim.x) n += p.flags[first + ci] != 0;
+        if (n) atomicAdd(&total, n);
+        __syncthreads();
+        if (threadIdx.x == 0) counts[t] = total;
+        __syncthreads();
+    }
+}
+
+// off[0..n] = exclusive prefix sums of counts[0..n-1]; one CTA
+__global__ void __launch_bounds__(1024) fix_scan_kernel(const unsigned *__restrict__ counts, unsigned *__restrict__ off, int n) {
+    __shared__ unsigned wsum[32];
+    __shared__ unsigned carry;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += 1024) {
+        const int i = base + tid;
+        const unsigned v = i < n ? counts[i] : 0u;
+        unsigned s = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, s, d);
+            if (lane >= d) s += o;
+        }
+        if (lane == 31) wsum[wid] = s;
+        __syncthreads();
+        if (wid == 0) {
+            unsigned ws = wsum[lane];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned o = __shfl_up_sync(0xffffffffu, ws, d);
+                if (lane >= d) ws += o;
+            }
+            wsum[lane] = ws;                                                // inclusive over the warps
+        }
+        __syncthreads();
+        const unsigned before = carry + (wid ? wsum[wid - 1] : 0u) + s - v;
+        if (i < n) off[i] = before;
+        __syncthreads();
+        if (tid == 1023) carry = before + v;
+        __syncthreads();
+    }
+    if (tid == 0) off[n] = carry;
+}
+
+__global__ void __launch_bounds__(128) fix_fill_kernel(const Params p, const BulkGeom g, const unsigned *__restrict__ off,
+                                                      uint2 *__restrict__ list) {
+    __shared__ unsigned cursor;
+    for (int t = blockIdx.x; t < g.n_tiles; t += gridDim.x) {
+        if (threadIdx.x == 0) cursor = 0;
+        __syncthreads();
+        const unsigned lo = off[t];
+        if (off[t + 1] != lo) {
+            const TileCoord c = tile_coord(t, g, p);
+            const int cells = c.rows * c.w;
+            const long long first = (long long)p.nx * (c.y + (long long)p.ny * c.z) + c.x0;
+            for (int ci = threadIdx.x; ci < cells; ci += blockDim.x) {
+                const unsigned fl = p.flags[first + ci];
+                if (fl != 0) list[lo + atomicAdd(&cursor, 1u)] = make_uint2((unsigned)ci | (fl << 16), p.bounce ? p.bounce[first + ci] : 0u);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Per-tile lists of flagged cells for the staged kernel's tile geometry g (Params::fix_off / fix_cells); p.flags
+// must hold the final flag bytes (FLAG_NEAR set).  The caller owns (cudaFree) both arrays.  Synchronises the stream.
+cudaError_t build_fix_lists_for(const Params &p, const BulkGeom &g, unsigned **off_out, uint2 **list_out, cudaStream_t st) {
+    *off_out = nullptr;
+    *list_out = nullptr;
+    unsigned *counts = nullptr, *off = nullptr;
+    uint2 *list = nullptr;
+    cudaError_t e = cudaMalloc((void **)&counts, (size_t)g.n_tiles * 4);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&off, ((size_t)g.n_tiles + 1) * 4);
+    const int grid = g.n_tiles < 148 * 32 ? g.n_tiles : 148 * 32;
+    unsigned total = 0;
+    if (e == cudaSuccess) {
+        fix_count_kernel<<<grid, 128, 0, st>>>(p, g, counts);
+        fix_scan_kernel<<<1, 1024, 0, st>>>(counts, off, g.n_tiles);
+        count_launch(2);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&total, off + g.n_tiles, 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&list, (size_t)(total ? total : 1) * sizeof(uint2));
+    if (e == cudaSuccess) {
+        fix_fill_kernel<<<grid, 128, 0, st>>>(p, g, off, list);
+        count_launch();
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (counts) cudaFree(counts);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (off) cudaFree(off);
+        if (list) cudaFree(list);
+        return e;
+    }
+    *off_out = off;
+    *list_out = list;
+    return cudaSuccess;
+}
+
 template <int F>
 __global__ void __launch_bounds__(256) encode_kernel(const float *__restrict__ x, unsigned short *__restrict__ c, long long n) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
@@ -171,26 +288,35 @@ __global__ void __launch_bounds__(512) enc_table_kernel(EncEntry *tab) {
     tab[idx] = e;
 }
 
+// The table of a format is built once per device, synchronously and under a lock: it is complete, and known to be, before
+// any caller on any stream gets its address (a flag set after an asynchronous launch would let a second handle on
+// another stream read a half-written table).  A failed build leaves the flag clear.
 cudaError_t enc_table(int fmt, const EncEntry **out, cudaStream_t st) {
+    static std::mutex mu;
     static bool built[64][7];
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || fmt < 0 || fmt > 6) return cudaErrorInvalidValue;
     EncEntry *base = nullptr;
     if ((e = cudaGetSymbolAddress((void **)&base, g_enc_tables)) != cudaSuccess) return e;
     EncEntry *tab = base + fmt * 512;
     *out = tab;
-    if (dev < 0 || dev >= 64 || fmt < 0 || fmt > 6) return cudaErrorInvalidValue;
+    if (fmt != F_P16_0S && fmt != F_P16_1S && fmt != F_P16_2C) return cudaSuccess;      // formats without a table
+    std::lock_guard<std::mutex> lock(mu);
     if (built[dev][fmt]) return cudaSuccess;
+    // cudaStreamSynchronize is not allowed while `st` is being captured into a graph: build on the legacy stream
+    (void)st;
     switch (fmt) {
-        case F_P16_0S: enc_table_kernel<F_P16_0S><<<1, 512, 0, st>>>(tab); break;
-        case F_P16_1S: enc_table_kernel<F_P16_1S><<<1, 512, 0, st>>>(tab); break;
-        case F_P16_2C: enc_table_kernel<F_P16_2C><<<1, 512, 0, st>>>(tab); break;
-        default: return cudaSuccess;                        // formats without a table
+        case F_P16_0S: enc_table_kernel<F_P16_0S><<<1, 512>>>(tab); break;
+        case F_P16_1S: enc_table_kernel<F_P16_1S><<<1, 512>>>(tab); break;
+        default: enc_table_kernel<F_P16_2C><<<1, 512>>>(tab); break;
     }
     count_launch();
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return e;
     built[dev][fmt] = true;
-    return cudaGetLastError();
+    return cudaSuccess;
 }
 
 // ---- pair codecs vs scalar codecs, exhaustively, on the device ----------------------------------------
@@ -261,6 +387,53 @@ cudaError_t launch_pair_selftest(int fmt, unsigned long long *mismatches_dev, cu
         case F_FP16: pair_selftest_kernel<F_FP16><<<blocks, 256, 0, st>>>(mismatches_dev, tab); break;
         default: return cudaErrorInvalidValue;
     }
+    count_launch();
+    return cudaGetLastError();
+}
+
+
+// ---- div3 (lbm_lattice.cuh) vs the compiler's IEEE division, on the device --------------------------------------
+// Denominators: every 2^7-th float in [2^-2, 2^2) and one pseudo-random float per index from all of [2^-60, 2^60];
+// numerators per denominator: +-0, pseudo-random multiples of the 16-bit formats' smallest steps (2^-39, 2^-25, 2^-21,
+// 2^-35, 2^-59), products k * b (exact quotients) and their FP32 neighbours, and pseudo-random floats of every
+// magnitude the guard's contract admits.  Every result must equal __fdiv_rn's bit for bit.
+__device__ __forceinline__ unsigned mix32(unsigned x) {
+    x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;
+    return x;
+}
+__global__ void __launch_bounds__(256) div_selftest_kernel(unsigned long long *mismatches) {
+    const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
+    unsigned long long bad = 0;
+    for (unsigned bi = gid; bi < (1u << 19); bi += n_threads) {
+        float bs[2];
+        bs[0] = __uint_as_float(0x3E800000u + (bi << 7));                               // [2^-2, 2^2)
+        bs[1] = __uint_as_float(0x21800000u + mix32(bi * 2654435761u + 17u) % (0x5D800000u - 0x21800000u));
+        for (int w = 0; w < 2; ++w) {
+            const float b = bs[w];
+            for (unsigned k = 0; k < 96; k += 3) {
+                float a[3], q[3];
+                for (unsigned m = 0; m < 3; ++m) {
+                    const unsigned h = mix32((bi * 96u + k + m) * 0x9E3779B9u + (unsigned)w);
+                    const unsigned kind = (k + m) % 8u, sel = (h >> 20) % 5u;
+                    float v;
+                    if (kind == 0) v = 0.0f;
+                    else if (kind == 1) v = ldexpf((float)(h & 0xFFFFFu), -39);          // the FP16S grid
+                    else if (kind == 2) v = ldexpf((float)(h & 0xFFFFu), sel == 0 ? -25 : sel == 1 ? -21 : sel == 2 ? -35 : -59);
+                    else if (kind == 3) v = __fmul_rn(b, (float)(int)(h & 0xFFFu));     // exact quotients (where the product is exact)
+                    else if (kind == 4) v = __uint_as_float(__float_as_uint(__fmul_rn(b, (float)(int)(1u + (h & 0xFFu)))) + (h >> 30));
+                    else v = __uint_as_float(0x13000000u + h % (0x5D800000u - 0x13000000u));  // 2^-89 .. 2^60
+                    a[m] = (h & 0x80000u) ? -v : v;
+                }
+                div3<1>(a, b, q, true);
+                for (int m = 0; m < 3; ++m) bad += __float_as_uint(q[m]) != __float_as_uint(__fdiv_rn(a[m], b));
+            }
+        }
+    }
+    if (bad) atomicAdd(mismatches, bad);
+}
+
+cudaError_t launch_div_selftest(unsigned long long *mismatches_dev, cudaStream_t st) {
+    div_selftest_kernel<<<148 * 8, 256, 0, st>>>(mismatches_dev);
     count_launch();
     return cudaGetLastError();
 }

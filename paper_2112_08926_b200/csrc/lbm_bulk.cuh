@@ -59,6 +59,10 @@ struct BulkGeom {
     FastDiv by_tpr, by_ytiles;
     FastDiv by_hw_full, by_hw_last;   // division by half the width of a full tile / of a row's last tile
     long long src_off[27]; // i*N - nx*(c_iy + ny*c_iz): source row of direction i relative to the own row, no wrap
+    // the same in BYTES, and the byte offset i*N*sizeof(element) of direction i (lbm_stage.cuh: the producer warps add
+    // them to a tile's base address with one uniform 64-bit add each)
+    long long src_boff[27], dir_boff[27];
+    int chunk_shift;       // lbm_stage.cuh: a tile has 2^chunk_shift chunk ids (>= its chunks of 32 cell pairs, >= 8)
 };
 
 // c_i of the library's numbering for a run-time direction index (copy issue only; the collision uses Lat<Q>)
@@ -80,6 +84,21 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned byt
 }
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// the same with a suspend-time hint: a waiting thread sleeps until the phase completes (or the hint, in ns, runs out)
+// instead of coming back to poll -- polling warps take issue slots from the arithmetic warps
+__device__ __forceinline__ void mbar_wait_sleepy(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LBM_WAITS_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+        "@p bra LBM_DONES_%=;\n"
+        "bra LBM_WAITS_%=;\n"
+        "LBM_DONES_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity), "r"(0x989680u)
+        : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
     asm volatile(

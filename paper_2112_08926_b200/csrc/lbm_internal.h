@@ -10,6 +10,7 @@
 namespace lbmk {
 
 constexpr int VARIANT_BULK = 16;      // LBM_VARIANT_BULK of include/lbm.h
+constexpr int VARIANT_STAGED = 32;    // LBM_VARIANT_STAGED of include/lbm.h
 
 struct UnitOps {
     // stream_collide: V = cells per thread (1, 2 or 4; nx % V == 0) of the per-thread kernel, or VARIANT_BULK
@@ -23,6 +24,10 @@ struct UnitOps {
                          cudaStream_t st);
     // FP64-arithmetic units only (lbm_unit64.cu), else null: read-out in double
     cudaError_t (*read64)(const void *A, const Params &p, bool force, double *rho, double *u, cudaStream_t st);
+    // warp-specialised staged kernel (lbm_stage.cuh; null in the FP64-arithmetic units): cells per tile, and the
+    // builder of the per-tile flagged-pair lists (Params::fix_off / fix_cells; the caller cudaFrees both)
+    int (*staged_tile_cells)();
+    cudaError_t (*build_fix_lists)(const Params &p, unsigned **off, uint2 **list, cudaStream_t st);
 };
 
 const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)
@@ -35,6 +40,9 @@ cudaError_t launch_codec(int fmt, bool encode, const void *in, void *out, long l
 struct EncEntry;
 cudaError_t enc_table(int fmt, const EncEntry **out, cudaStream_t st);   // device pointer to the format's encoder table (built on first use)
 cudaError_t launch_pair_selftest(int fmt, unsigned long long *mismatches_dev, cudaStream_t st);
+cudaError_t launch_div_selftest(unsigned long long *mismatches_dev, cudaStream_t st);
+struct BulkGeom;
+cudaError_t build_fix_lists_for(const Params &p, const BulkGeom &g, unsigned **off, uint2 **list, cudaStream_t st);
 
 void count_launch(long long n = 1);
 

@@ -3,6 +3,9 @@
 #include "lbm_internal.h"
 #include "lbm_kernels.cuh"
 #include "lbm_bulk.cuh"
+#include "lbm_stage.cuh"
+
+#include <mutex>
 
 #ifndef LBM_Q
 #error "compile with -DLBM_Q=<velocity set> -DLBM_F=<format>"
@@ -51,26 +54,47 @@ BulkGeom bulk_geom(const Params &p, long long *tiles) {
     g.n_tiles = (int)(*tiles < 0x7FFFFFFFLL ? *tiles : 0x7FFFFFFFLL);
     g.by_tpr = FastDiv::make(g.tiles_per_row);
     g.by_ytiles = FastDiv::make(g.ytiles);
-    for (int i = 0; i < 27; ++i)
+    for (int i = 0; i < 27; ++i) {
         g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
+        g.src_boff[i] = g.dir_boff[i] = 0;                   // lbm_stage.cuh only
+    }
+    g.chunk_shift = 0;
     return g;
+}
+
+// Resident CTAs of a persistent kernel on the CURRENT device (SMs x CTAs per SM), and the opt-in to its dynamic shared
+// memory.  Both are per-device state: resolved once per device and kernel, under a lock.  `cache` is the calling
+// launcher's own table (one per kernel instantiation).
+struct CtaCache {
+    std::mutex mu;
+    int ctas[64] = {};
+};
+template <class K>
+cudaError_t resident_ctas(K kern, int threads, int smem, int *out, CtaCache &cache) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(cache.mu);
+    if (cache.ctas[dev] == 0) {
+        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+        int sms = 0, per_sm = 0;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem)) != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        cache.ctas[dev] = sms * per_sm;
+    }
+    *out = cache.ctas[dev];
+    return cudaSuccess;
 }
 
 template <bool FORCE, int COLL = 0>
 cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st) {
     typedef BulkShape<Q, F, BULK_NT> SH;
     auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, FORCE, COLL>;
-    static int ctas = 0;                      // resident CTAs on the device, resolved once per instantiation
-    if (ctas == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SH::SMEM);
-        if (e != cudaSuccess) return e;
-        int dev = 0, sms = 0, per_sm = 0;
-        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BULK_NT, SH::SMEM)) != cudaSuccess) return e;
-        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-        ctas = sms * per_sm;
-    }
+    int ctas = 0;
+    static CtaCache cache;                    // one per instantiation of this launcher
+    if (cudaError_t e = resident_ctas(kern, BULK_NT, SH::SMEM, &ctas, cache)) return e;
     long long tiles = 0;
     const BulkGeom g = bulk_geom(p, &tiles);
     if (p.nx % 16 != 0 || tiles > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
@@ -85,7 +109,66 @@ cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st
     return cudaGetLastError();
 }
 
+// ---- the warp-specialised staged variant (lbm_stage.cuh) ----------------------------------------------
+BulkGeom stage_geom(const Params &p, long long *tiles) {
+    typedef StageShape<Q, F> SH;
+    BulkGeom g;
+    g.tile_w = p.nx <= SH::TC ? p.nx : SH::TC;
+    g.tiles_per_row = (p.nx + g.tile_w - 1) / g.tile_w;
+    g.rows_per_tile = g.tiles_per_row == 1 ? SH::TC / p.nx : 1;
+    const int w_last = p.nx - (g.tiles_per_row - 1) * g.tile_w;
+    g.by_hw_full = FastDiv::make(g.tile_w / 2);
+    g.by_hw_last = FastDiv::make(w_last / 2);
+    g.ytiles = (p.ny + g.rows_per_tile - 1) / g.rows_per_tile;
+    *tiles = (long long)g.tiles_per_row * g.ytiles * p.nz;
+    g.n_tiles = (int)(*tiles < 0x7FFFFFFFLL ? *tiles : 0x7FFFFFFFLL);
+    g.by_tpr = FastDiv::make(g.tiles_per_row);
+    g.by_ytiles = FastDiv::make(g.ytiles);
+    for (int i = 0; i < 27; ++i) {
+        g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
+        g.src_boff[i] = g.src_off[i] * SH::ES;
+        g.dir_boff[i] = i < Q ? (long long)i * p.N * SH::ES : 0;
+    }
+    const int chunks_full = (g.rows_per_tile * (g.tile_w / 2) + 31) / 32;
+    g.chunk_shift = 3;
+    while ((1 << g.chunk_shift) < chunks_full) ++g.chunk_shift;
+    return g;
+}
+
+template <bool FORCE, int COLL = 0>
+cudaError_t launch_staged(const void *A, void *B, const Params &p, cudaStream_t st) {
+    typedef StageShape<Q, F> SH;
+    auto kern = stream_collide_staged_kernel<Q, F, FORCE, COLL>;
+    static CtaCache cache;
+    int ctas = 0;
+    if (cudaError_t e = resident_ctas(kern, SH::NT, SH::SMEM, &ctas, cache)) return e;
+    long long tiles = 0;
+    const BulkGeom g = stage_geom(p, &tiles);
+    if (p.nx % 16 != 0 || tiles >= 0x7FFFFFFFLL) return cudaErrorInvalidValue;
+    const int grid = (int)(tiles < ctas ? tiles : ctas);
+    const EncEntry *tab = nullptr;
+    if (PairCodec<F>::TABLE) {
+        cudaError_t e = enc_table(F, &tab, st);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<grid, SH::NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g, tab);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// Per-tile lists of flagged cell pairs for this unit's tile geometry (lbm_aux.cu)
+cudaError_t build_fix_lists(const Params &p, unsigned **off_out, uint2 **list_out, cudaStream_t st) {
+    long long tiles = 0;
+    const BulkGeom g = stage_geom(p, &tiles);
+    if (p.nx % 16 != 0 || tiles >= 0x7FFFFFFFLL) return cudaErrorInvalidValue;
+    return build_fix_lists_for(p, g, off_out, list_out, st);
+}
+
 cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
+    if (V == VARIANT_STAGED) {
+        if (coll == 1) return force ? launch_staged<true, 1>(A, B, p, st) : launch_staged<false, 1>(A, B, p, st);
+        return force ? launch_staged<true>(A, B, p, st) : launch_staged<false>(A, B, p, st);
+    }
     if (coll == 1) {
         // TRT (R13): the staged kernel, or the per-thread kernel with one, two or four cells per thread
         if (V == VARIANT_BULK) return force ? launch_bulk<true, 1>(A, B, p, st) : launch_bulk<false, 1>(A, B, p, st);
@@ -133,6 +216,13 @@ cudaError_t probe(const void *A, const Params &p, bool force, const long long *c
 }
 
 const char *name(int V, int coll, bool force) {
+    if (V == VARIANT_STAGED) {
+        if (coll == 1)
+            return force ? "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
+                         : "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0,COLL=TRT>";
+        return force ? "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1>"
+                     : "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0>";
+    }
     if (coll == 1) {
         if (V == VARIANT_BULK)
             return force ? "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
@@ -159,10 +249,11 @@ const char *name(int V, int coll, bool force) {
 }
 
 int bulk_tile_cells() { return 2 * BULK_NT; }
+int staged_tile_cells() { return StageShape<Q, F>::TC; }
 
 }  // namespace
 
 extern const UnitOps LBM_UNIT_SYMBOL;
-const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells, probe};
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells, probe, nullptr, staged_tile_cells, build_fix_lists};
 
 }  // namespace lbmk

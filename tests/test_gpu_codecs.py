@@ -67,6 +67,15 @@ def test_roundtrip_on_device(name):
     assert np.array_equal(lbm.codec_encode(name, lbm.codec_decode(name, finite)), finite)
 
 
+def test_corner_thresholds_on_device():
+    """The class-B corner vectors (tests/golden/codec_corner_vectors.txt) through the device encoders."""
+    from .test_oracle_codecs import corner_vectors
+    for name, x, at, below in corner_vectors():
+        lo = np.nextafter(x, np.float32(0))
+        got = lbm.codec_encode(name, np.array([x, lo, -x, -lo], np.float32))
+        assert [int(c) for c in got] == [at, below, at | 0x8000, below | 0x8000], (name, float(x), [hex(int(c)) for c in got])
+
+
 def test_codec_edge_cases():
     assert lbm.codec_encode("FP16C", np.zeros(0, np.float32)).size == 0
     with pytest.raises(lbm.LbmError):
@@ -78,3 +87,9 @@ def test_pair_codecs_equal_scalar_codecs_exhaustively(name):
     """The staged kernel's converters (PairCodec) vs the scalar ones (compared with the oracle above): all 65 536
     codes and all 2^32 FP32 bit patterns, on the device."""
     assert lbm.codec_pair_selftest(name) == 0
+
+
+def test_shared_division_equals_ieee_division():
+    """The staged kernel's u = j / rho with one shared reciprocal (div3) vs __fdiv_rn, ~10^8 pairs incl. signed zero
+    numerators, on the device."""
+    assert lbm.div_selftest() == 0

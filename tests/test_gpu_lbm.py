@@ -154,7 +154,7 @@ BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16
                (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1))]
 
 
-STAGED = [(lbm.VARIANT_BULK, "bulk")]
+STAGED = [(lbm.VARIANT_BULK, "bulk"), (lbm.VARIANT_STAGED, "staged")]
 
 
 @pytest.mark.parametrize("q,shape", BULK_SHAPES)
@@ -195,11 +195,14 @@ def test_automatic_variant_choice():
     w = wl.perturbed_equilibrium(256, 64, 64, seed=2)
     g16 = lbm.from_workload(w, "FP16S")
     g32 = lbm.from_workload(w, "FP32")
-    assert "bulk" in g16.kernel_name and "bulk" not in g32.kernel_name
+    assert "staged" in g16.kernel_name and "stream_collide_kernel" in g32.kernel_name
+    w = wl.random_walls(w, 0.01, seed=3)                    # flagged cells: the staged kernel for FP32 storage too
+    assert "staged" in lbm.from_workload(w, "FP32").kernel_name
     w = wl.perturbed_equilibrium(36, 2, 2, seed=2)          # rows not 16-cell aligned: per-thread kernel
-    assert "bulk" not in lbm.from_workload(w, "FP16S").kernel_name
-    with pytest.raises(lbm.LbmError):
-        lbm.from_workload(w, "FP16S", variant=lbm.VARIANT_BULK)
+    assert "stream_collide_kernel" in lbm.from_workload(w, "FP16S").kernel_name
+    for v in (lbm.VARIANT_BULK, lbm.VARIANT_STAGED):
+        with pytest.raises(lbm.LbmError):
+            lbm.from_workload(w, "FP16S", variant=v)
 
 
 # ---- BASELINE.json's full size, in the launch configuration bench.py times ---------------------------
@@ -226,7 +229,7 @@ def _block(field, origin, L):
 def test_full_size_sampled_blocks(full_size_workload, name):
     w, L = full_size_workload, FULL_L
     g = lbm.from_workload(w, name)
-    assert ("bulk" in g.kernel_name) == (name != "FP32")
+    assert ("staged" in g.kernel_name) == (name != "FP32")
     g.step(FULL_STEPS)
     grho, gu = g.read_rho_u()
     g.close()
@@ -264,7 +267,7 @@ def test_full_size_mass_conservation(full_size_workload):
 
 # ---- equilibrium boundary cells (LBM_FLAG_EQ, R15) and the Karman set-up of BASELINE configs[3] ----
 EQ_CASES = [(q, shape, v) for q, shape in [(19, (24, 9, 7)), (19, (272, 6, 5)), (27, (32, 7, 5)), (9, (48, 13, 1))]
-            for v in (1, 2, lbm.VARIANT_BULK) if v != lbm.VARIANT_BULK or shape[0] % 16 == 0]
+            for v in (1, 2, lbm.VARIANT_BULK, lbm.VARIANT_STAGED) if v < 16 or shape[0] % 16 == 0]
 
 
 @pytest.mark.parametrize("q,shape,variant", EQ_CASES)

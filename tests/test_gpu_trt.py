@@ -101,17 +101,18 @@ def test_trt_periodic_without_force(name):
     assert_parity(osim, gsim, name)
 
 
-# ---- staged kernel (lbm_bulk.cuh): one tile per row, several tiles with a ragged last tile, D3Q27, D2Q9 -----
+# ---- staged kernels (lbm_bulk.cuh, lbm_stage.cuh): one tile per row, several tiles with a ragged last tile, D3Q27, D2Q9 -----
 @pytest.mark.parametrize("q,shape", [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 3, 2)), (27, (272, 3, 3)), (9, (1056, 3, 1))])
 @pytest.mark.parametrize("name", ALL_FORMATS)
 @pytest.mark.parametrize("walls", [False, True])
-def test_trt_staged_kernel(q, shape, name, walls):
+@pytest.mark.parametrize("variant,tag", [(lbm.VARIANT_BULK, "bulk"), (lbm.VARIANT_STAGED, "staged")])
+def test_trt_staged_kernel(q, shape, name, walls, variant, tag):
     w = wl.perturbed_equilibrium(*shape, seed=53, velset=q, tau=0.7)
     if walls:
         w = wl.random_walls(w, 0.12, seed=59, moving_fraction=0.5)
         w.force = (1e-5, -2e-5, 0.0 if q == 9 else 3e-5)
-    osim, gsim = run_pair(w, name, 16, variant=lbm.VARIANT_BULK)
-    assert "bulk" in gsim.kernel_name
+    osim, gsim = run_pair(w, name, 16, variant=variant)
+    assert tag in gsim.kernel_name
     assert_parity(osim, gsim, name)
 
 
@@ -124,9 +125,10 @@ def test_trt_lid_driven_cavity_small(name):
 
 
 @pytest.mark.parametrize("name", ["FP32", "FP16C"])
-def test_trt_equilibrium_boundary_cells(name):
+@pytest.mark.parametrize("variant", [lbm.VARIANT_BULK, lbm.VARIANT_STAGED])
+def test_trt_equilibrium_boundary_cells(name, variant):
     w = wl.equilibrium_rim(wl.perturbed_equilibrium(48, 7, 5, seed=61, tau=0.65))
-    osim, gsim = run_pair(w, name, 20, variant=lbm.VARIANT_BULK)
+    osim, gsim = run_pair(w, name, 20, variant=variant)
     assert_parity(osim, gsim, name)
 
 
@@ -151,7 +153,7 @@ def _block(field, origin, L):
 def test_trt_full_size_sampled_blocks(full_size_workload, name):
     w, L = full_size_workload, FULL_L
     g = lbm.from_workload(w, name, collision=lbm.TRT)
-    assert "COLL=TRT" in g.kernel_name and ("bulk" in g.kernel_name) == (name != "FP32")
+    assert "COLL=TRT" in g.kernel_name and ("staged" in g.kernel_name) == (name != "FP32")
     g.step(FULL_STEPS)
     grho, gu = g.read_rho_u()
     g.close()

@@ -207,3 +207,38 @@ def test_posit_accuracy_intervals():
         assert counts[posit][lo - 1] < counts[other][lo - 1], (posit, other, "below", lo)
         if hi < 1:
             assert counts[posit][hi] < counts[other][hi], (posit, other, "above", hi)
+
+
+def corner_vectors():
+    """tests/golden/codec_corner_vectors.txt -> [(format, x at the threshold (float32), code at, code just below)]"""
+    out = []
+    for line in open(os.path.join(GOLDEN, "codec_corner_vectors.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, scale, t, at, below = line.split()
+        mant, exp = t.split("*2^")
+        x = np.float64(mant) * 2.0 ** int(exp) / float(scale)
+        assert np.float64(np.float32(x)) == x, (name, t)          # every threshold is an FP32 number
+        out.append((name, np.float32(x), int(at, 16), int(below, 16)))
+    return out
+
+
+def test_corner_thresholds():
+    """Class-B corners (R14): the first codes above zero and the step into the saturating code, exactly at
+    the midpoints the value tables fix and one FP32 step below them, both signs -- the regions test_listing1_encode
+    has to mask out because the listing is not nearest-value there."""
+    for name, x, at, below in corner_vectors():
+        fmt = FORMATS[name]
+        lo = np.nextafter(x, np.float32(0))
+        got = oracle.encode(fmt, np.array([x, lo, -x, -lo], np.float32))
+        assert [int(c) for c in got] == [at, below, at | 0x8000, below | 0x8000], (name, float(x), [hex(int(c)) for c in got])
+    # beyond the largest number every software format saturates (PAPER.md:816, 844); zero keeps its sign
+    for name in SOFT:
+        got = oracle.encode(FORMATS[name], np.array([3.0, 1e30, np.inf, -1e30, 0.0, -0.0], np.float32))
+        big = 0x7FFF
+        if name in ("P16_0S", "P16_1S"):
+            assert int(got[0]) < big                                # 3 is inside their range
+            got = got[1:]
+            assert [int(c) for c in got] == [big, big, big | 0x8000, 0, 0x8000], name
+        else:
+            assert [int(c) for c in got] == [big, big, big, big | 0x8000, 0, 0x8000], name
