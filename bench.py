@@ -9,7 +9,14 @@ storage format and achieved HBM GB/s vs the measured peak.  The JSON line's `val
 format (FP16S, the paper's fastest); every format is listed under `formats`.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--size L] [--formats FP32,FP16S,...]
+    python bench.py --workload cavity|poiseuille|karman [--size L]   # the boxes with boundaries of configs[1..3]
     python bench.py --impl reference     # the CPU oracle, as it stands, on a bounded sample
+
+--workload periodic (default) is the headline.  The others time the same lbm_step on the set-ups of BASELINE.json
+configs[2] (lid-driven cavity L^3, default 256), configs[1] (Poiseuille channel L^3 with walls on the y faces and a
+body force, default 256) and configs[3] (Karman street 4L x L x L/4 with a cylinder and an equilibrium rim, default
+L = 256, i.e. 1024 x 256 x 64), inputs from workloads/: same JSON line, same roofline accounting (2 q s + 1 bytes per
+cell), clocks and cpu_baseline.
 
 N > 1 (torchrun): the path does not exchange data between GPUs in this tier:
 every rank runs an independent replica of the box ("weak" scaling), timed as the max over ranks.
@@ -48,19 +55,21 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
 
 
-def recorded_traffic(fmt_name, size):
+def recorded_traffic(fmt_name, size, workload="periodic"):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the stream_collide kernel from the
-    committed `ncu --set full` capture: profiles/dram_traffic.csv, columns velset,format,L,bytes_per_launch,profile.
-    The LAST matching row wins (newest profile).  None if no capture exists for this format / size."""
+    committed `ncu --set full` captures: profiles/dram_traffic.csv, columns velset,format,L,bytes_per_launch,profile
+    [,workload].  The value is RECORDED, not measured in this run (ncu cannot run inside a timed region): the line
+    carries the profile id beside it.  The LAST matching row wins (newest profile).  (None, None) if no capture
+    exists for this format / size / workload."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
-        return None
-    found = None
+        return None, None
+    found = (None, None)
     for line in open(path):
         p = [c.strip() for c in line.split(",")]
-        if len(p) >= 4 and p[0] == "D3Q19" and p[1] == fmt_name and p[2] == str(size):
+        if len(p) >= 5 and p[0] == "D3Q19" and p[1] == fmt_name and p[2] == str(size) and (p[5] if len(p) > 5 else "periodic") == workload:
             try:
-                found = float(p[3])
+                found = (float(p[3]), p[4])
             except ValueError:
                 pass
     return found
@@ -147,6 +156,26 @@ def rank_seed(rank):
     return SEED + rank
 
 
+def make_workload(kind, L, Q, seed):
+    """The synthetic input of one rank: a workloads.Workload and a one-line description."""
+    nz = 1 if Q == 9 else L
+    if kind == "periodic":
+        w = wl.perturbed_equilibrium(L, L, nz, seed=seed, tau=TAU, velset=Q)
+        what = (f"configs[4] bandwidth sweep: D{2 if Q == 9 else 3}Q{Q} periodic {'square' if Q == 9 else 'cube'} "
+                f"{L}^{2 if Q == 9 else 3}, perturbed equilibrium (seed {SEED}), tau {TAU}")
+    elif kind == "cavity":
+        w = wl.lid_driven_cavity(L, velset=Q)
+        what = f"configs[2] lid-driven cavity {L}^3, wall shell, lid u = 0.1, Re = 1000 (tau {w.tau:.4f}), fluid at rest"
+    elif kind == "poiseuille":
+        w = wl.poiseuille_channel(L, L, L, velset=Q)
+        what = f"configs[1] Poiseuille channel {L}^3, walls on the y faces, Guo force, tau {w.tau}, fluid at rest"
+    else:
+        w = wl.karman_vortex_street(4 * L, L, max(L // 4, 1), radius=L / 16.0, velset=Q)
+        what = (f"configs[3] Karman street {w.nx}x{w.ny}x{w.nz}, cylinder R = {L / 16.0:g}, equilibrium rim u = 0.05, "
+                f"Re = 200 (tau {w.tau:.4f})")
+    return w, what
+
+
 def run_ours(args):
     import torch
 
@@ -157,24 +186,34 @@ def run_ours(args):
     dist = None
     if world > 1:
         import torch.distributed as dist
-    L, K, W, Q = args.size, args.steps, args.warmup, args.velset
-    nz = 1 if Q == 9 else L
-    N = L * L * nz
+    K, W, Q, kind = args.steps, args.warmup, args.velset, args.workload
+    L = args.size if args.size else (512 if kind == "periodic" else 256)
     formats = args.formats.split(",")
+    if kind != "periodic":
+        formats = [f for f in formats if not f.startswith("FP64")] or formats
     peak, peak_src = measured_peak()
 
-    # synthetic input.  Default: the seeded host arrays of workloads.perturbed_equilibrium, pinned (they are the
-    # end-to-end leg's input) and copied to the device.  --device-init (sweep sizes whose host arrays would be
-    # tens of GB): the same recipe drawn on the device by torch's seeded generator; no end-to-end leg then.
-    host_input = not args.device_init
+    # synthetic input.  Default: the seeded host arrays of workloads/, pinned (they are the end-to-end leg's input)
+    # and copied to the device.  --device-init (periodic sweep sizes whose host arrays would be tens of GB): the same
+    # recipe drawn on the device by torch's seeded generator; no end-to-end leg then.
+    host_input = not (args.device_init and kind == "periodic")
+    flags, force = None, None
     if host_input:
-        w = wl.perturbed_equilibrium(L, L, nz, seed=rank_seed(rank), tau=TAU, velset=Q)
+        w, what = make_workload(kind, L, Q, rank_seed(rank))
+        nx, ny, nz, tau = w.nx, w.ny, w.nz, w.tau
+        N = w.n_cells
+        flags = w.flags if w.flags.any() else None
+        force = w.force if any(float(v) != 0.0 for v in w.force) else None
         rho_h = torch.from_numpy(w.rho).pin_memory()
         u_h = torch.from_numpy(w.u).pin_memory()
         rho_d, u_d = rho_h.cuda(), u_h.cuda()
         rho_out = torch.empty(N, dtype=torch.float32).pin_memory()
         u_out = torch.empty((3, N), dtype=torch.float32).pin_memory()
     else:
+        nx, ny, nz, tau = L, L, (1 if Q == 9 else L), TAU
+        N = nx * ny * nz
+        what = (f"configs[4] bandwidth sweep: D{2 if Q == 9 else 3}Q{Q} periodic {'square' if Q == 9 else 'cube'} "
+                f"{L}^{2 if Q == 9 else 3}, perturbed equilibrium drawn on the device (seed {SEED}), tau {TAU}")
         gen = torch.Generator(device="cuda").manual_seed(rank_seed(rank))
         rho_d = 1.0 + 1e-3 * torch.randn(N, device="cuda", generator=gen)
         u_d = (0.05 / 3 ** 0.5) * (2.0 * torch.rand((3, N), device="cuda", generator=gen) - 1.0)
@@ -194,8 +233,10 @@ def run_ours(args):
 
     results, launches_total = {}, 0
     for name in formats:
-        sim = lbm.Simulation(L, L, nz, Q, name, TAU, cells_per_thread=args.cells_per_thread,
+        sim = lbm.Simulation(nx, ny, nz, Q, name, tau, force=force, cells_per_thread=args.cells_per_thread,
                              collision=lbm.TRT if args.collision == "TRT" else lbm.BGK)
+        if flags is not None:
+            sim.set_flags(flags)
         sim.init(rho_d, u_d)
         sim.step(W)
         barrier()
@@ -238,20 +279,24 @@ def run_ours(args):
     head = HEADLINE if HEADLINE in results else formats[0]
     r = results[head]
     clocks = sampler.summary(windows)
+    traffic, prof = recorded_traffic(head, L, kind) if Q == 19 else (None, None)
+    traffic_src = (f"recorded: ncu --set full capture profiles/{prof} (dram__bytes_read.sum + dram__bytes_write.sum of one launch), "
+                   "not measured in this run") if traffic else None
     line = {
         "metric": METRIC, "value": r["mlups"], "unit": "MLUPs/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"configs[4] bandwidth sweep: D{2 if Q == 9 else 3}Q{Q} {args.collision} periodic {'square' if Q == 9 else 'cube'} {L}^{2 if Q == 9 else 3}, perturbed equilibrium "
-                               f"(seed {SEED}), tau {TAU}, headline storage format {head}",
+        "config": {"workload": f"{what}; {args.collision}; headline storage format {head}",
                    "cells": N, "l2_policy": "inputs larger than L2 (two DDF buffers of "
-                                            f"{N * Q * (4 if head == 'FP32' else 2) / 1e9:.1f} GB each, no flush needed)",
+                                            f"{N * Q * (4 if head == 'FP32' else 2) / 1e9:.2f} GB each, no flush needed)"
+                                            if 2 * N * Q * (4 if head == 'FP32' else 2) > 2.5e8 else
+                                            "box smaller than twice the 126 MB L2: partly L2-resident, not a roofline quote",
                    "parallelism": f"{world} independent replica(s)"},
         "formats": results,
         "speedup_16bit_vs_fp32": (round(results[head]["mlups"] / results["FP32"]["mlups"], 3)
                                   if "FP32" in results and head != "FP32" else None),
         "roofline": {"bound": "hbm", "kernel": r["kernel"], "achieved": r["hbm_gbs"], "peak": peak, "unit": "GB/s",
-                     "frac": r["frac_of_peak"], "traffic": recorded_traffic(head, L) if Q == 19 else None, "peak_source": peak_src,
+                     "frac": r["frac_of_peak"], "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": N * r["bytes_per_cell"]},
         "e2e": {"value": r["e2e_mlups"], "unit": "MLUPs/s", "h2d_bytes_per_step": 16 * N / K,
                 "d2h_bytes_per_step": 16 * N / K,
@@ -259,17 +304,28 @@ def run_ours(args):
         "gpu_launches": launches_total, "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(head, budget_s=args.cpu_seconds, collision=args.collision)
+        line["cpu_baseline"] = cpu_baseline(head, budget_s=args.cpu_seconds, collision=args.collision, kind=kind)
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
 
 
-def oracle_run(fmt_name, L, steps, warmup, collision="BGK"):
-    """Time the CPU oracle, as it stands, on an L^3 sample of the workload.  Returns (mlups, cores, seconds)."""
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_run(fmt_name, L, steps, warmup, collision="BGK", kind="periodic", threads=0):
+    """Time the CPU oracle, as it stands, on a sample of the workload with edge L (see make_workload).
+    Returns (mlups, cores, seconds, cells)."""
     import oracle
-    cores = oracle.set_threads(os.cpu_count() or 1)
-    w = wl.perturbed_equilibrium(L, L, L, seed=SEED, tau=TAU)
+    cores = oracle.set_threads(threads or os.cpu_count() or 1)
+    w, _ = make_workload(kind, L, 19, SEED)
     sim = oracle.from_workload(w, wl.FORMATS[fmt_name])
     if collision == "TRT":
         sim.set_collision(oracle.TRT)
@@ -277,18 +333,23 @@ def oracle_run(fmt_name, L, steps, warmup, collision="BGK"):
     t0 = time.perf_counter()
     sim.step(steps)
     dt = time.perf_counter() - t0
-    return L ** 3 * steps / dt / 1e6, cores, dt
+    return w.n_cells * steps / dt / 1e6, cores, dt, w.n_cells
 
 
-def cpu_baseline(fmt_name, budget_s=15.0, collision="BGK"):
-    """The oracle on a BOUNDED sample: a 128^3 periodic box of the same recipe (beyond the LLC), step
-    count sized from a 1-step probe so that the timed part takes about `budget_s` seconds."""
-    L = 128
-    probe, cores, dt = oracle_run(fmt_name, L, 1, 1, collision)
-    steps = max(2, min(200, int(budget_s / max(dt, 1e-3))))
-    mlups, cores, dt = oracle_run(fmt_name, L, steps, 0, collision)
+def cpu_baseline(fmt_name, budget_s=15.0, collision="BGK", kind="periodic"):
+    """The oracle on a BOUNDED sample of the same workload (128^3 periodic / cavity / channel, 256 x 64 x 16 Karman
+    box: beyond the LLC), on all host cores and on one, step counts sized from a 1-step probe so that the two timed
+    parts take about `budget_s` seconds together."""
+    L = 64 if kind == "karman" else 128
+    probe, cores, dt, cells = oracle_run(fmt_name, L, 1, 1, collision, kind)
+    steps = max(2, min(200, int(0.6 * budget_s / max(dt, 1e-3))))
+    mlups, cores, dt, cells = oracle_run(fmt_name, L, steps, 0, collision, kind)
+    steps1 = max(1, min(50, int(0.4 * budget_s / max(dt / steps * cores, 1e-3))))
+    mlups1, _, dt1, _ = oracle_run(fmt_name, L, steps1, 0, collision, kind, threads=1)
     return {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle",
-            "sample": f"D3Q19 {collision} {fmt_name} storage, {L}^3 periodic box of the same recipe, {steps} steps, {dt:.1f} s"}
+            "one_core": round(mlups1, 2), "cpu_model": cpu_model(),
+            "sample": f"D3Q19 {collision} {fmt_name} storage, {kind} box of {cells} cells of the same recipe, "
+                      f"{steps} steps in {dt:.1f} s on {cores} threads, {steps1} steps in {dt1:.1f} s on one"}
 
 
 def run_reference(args):
@@ -297,10 +358,10 @@ def run_reference(args):
         return
     K, W = args.steps, args.warmup
     L = 128
-    probe, cores, dt1 = oracle_run(HEADLINE, L, 1, 0, args.collision)
+    probe, cores, dt1, _ = oracle_run(HEADLINE, L, 1, 0, args.collision)
     K_eff = max(1, min(K, int(120.0 / max(dt1, 1e-3))))       # keep the whole run within a few minutes
-    mlups, cores, dt = oracle_run(HEADLINE, L, K_eff, min(W, 2), args.collision)
-    sample = (f"D3Q19 {args.collision} {HEADLINE} storage, {L}^3 periodic sample box of the {args.size}^3 workload, "
+    mlups, cores, dt, _ = oracle_run(HEADLINE, L, K_eff, min(W, 2), args.collision)
+    sample = (f"D3Q19 {args.collision} {HEADLINE} storage, {L}^3 periodic sample box of the {args.size or 512}^3 workload, "
               f"{K_eff} timed steps, {dt:.1f} s, {cores} OpenMP threads")
     line = {"impl": "reference", "metric": METRIC, "value": round(mlups, 2), "unit": "MLUPs/s",
             "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": K_eff, "warmup": min(W, 2),
@@ -309,7 +370,8 @@ def run_reference(args):
             "config": {"workload": f"configs[4] bandwidth sweep: D3Q19 {args.collision} periodic cube, perturbed equilibrium "
                                    f"(seed {SEED}), tau {TAU}, storage format {HEADLINE}; CPU oracle on a bounded sample",
                        "sample": sample},
-            "cpu_baseline": {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": round(mlups, 2), "unit": "MLUPs/s", "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model()},
             "e2e": {"value": round(mlups, 2), "unit": "MLUPs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -321,7 +383,9 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--size", type=int, default=512, help="cube edge L")
+    ap.add_argument("--size", type=int, default=0, help="cube edge L (default 512; 256 for the boxes with boundaries)")
+    ap.add_argument("--workload", default="periodic", choices=["periodic", "cavity", "poiseuille", "karman"],
+                    help="periodic = the headline (configs[4]); the others: the boxes with boundaries of configs[1..3]")
     ap.add_argument("--formats", default="FP32,FP16S,FP16C,P16_0S,P16_1S,P16_2C,FP64,FP64_FP32")
     ap.add_argument("--velset", type=int, default=19, choices=[9, 19, 27], help="sweep only; the headline is D3Q19")
     ap.add_argument("--device-init", action="store_true", help="draw the input on the device (big sweep sizes)")

@@ -88,10 +88,9 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream);
  * bit for bit).
  *   LBM_VARIANT_AUTO   the library chooses;
  *   1, 2, 4            the per-thread kernel with that many cells per thread along x (nx a multiple of it);
- *   LBM_VARIANT_BULK   the shared-memory-staged kernel: DDF rows move by cp.async.bulk, persistent CTAs
- *                      (nx a multiple of 16);
- *   LBM_VARIANT_STAGED the warp-specialised staged kernel: one producer warp per CTA moves loads AND stores with
- *                      cp.async.bulk, the other warps only compute (nx a multiple of 16).
+ *   LBM_VARIANT_STAGED the shared-memory-staged kernel: persistent CTAs, one loader and one storer warp move every
+ *                      DDF with cp.async.bulk, the other warps only compute (nx a multiple of 16).
+ *                      LBM_VARIANT_BULK is the same kernel (the name of its first version).
  * lbm_set_cells_per_thread(h, v) = lbm_set_variant(h, v) restricted to v in {0, 1, 2, 4}. */
 enum { LBM_VARIANT_AUTO = 0, LBM_VARIANT_BULK = 16, LBM_VARIANT_STAGED = 32 };
 int lbm_set_variant(lbm_t *h, int variant);

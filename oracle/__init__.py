@@ -36,6 +36,7 @@ def lib():
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_destroy.restype = None
         L.orc_set_collision.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.orc_set_shifting.argtypes = [C.c_void_p, C.c_int]
         for name in ("orc_set_flags",):
             getattr(L, name).argtypes = [C.c_void_p, C.c_void_p]
         for name in ("orc_init", "orc_init_f64", "orc_read_rho_u", "orc_read_rho_u_f64"):
@@ -141,6 +142,10 @@ class Sim:
     def set_collision(self, collision, lam=3.0 / 16.0):
         assert lib().orc_set_collision(self._h, int(collision), float(lam)) == 0
 
+    def set_shifting(self, on: bool):
+        """DDF-shifting on (default) / off (eqs (19)-(23), the paper's negative control); call before init"""
+        assert lib().orc_set_shifting(self._h, 1 if on else 0) == 0
+
     def step(self, n=1):
         assert lib().orc_step(self._h, int(n)) == 0
 
@@ -164,8 +169,10 @@ class Sim:
         return lib().orc_sum_ddf(self._h)
 
 
-def from_workload(w, fmt=FP32, arith=ARITH_F32) -> Sim:
+def from_workload(w, fmt=FP32, arith=ARITH_F32, shifted=True) -> Sim:
     s = Sim(w.nx, w.ny, w.nz, w.velset, fmt, w.tau, w.force, arith)
+    if not shifted:
+        s.set_shifting(False)
     s.set_flags(w.flags)
     s.init(w.rho, w.u)
     return s

@@ -14,6 +14,10 @@
 //   R8  f_i^B(x) = fma(1-omega, f_i^temp, omega f_i^eq)                        eq (28)
 //   R10 Guo forcing source term (named at PAPER.md:233, formula: DESIGN.md R10)
 //   R15 equilibrium boundary cells (named at PAPER.md:322): never updated, they keep f^eq(rho0, u0) from init
+//   R17 the same step WITHOUT DDF-shifting, eqs (19)-(23), the paper's negative control (dashed curves,
+//       PAPER.md:265, 316): the stored quantity is f_i, rho = sum f_i (no "+1"), f^eq by eq (22)
+//   R18 zero-gradient outflow cells (BASELINE configs[3]; NOT in the paper: DESIGN.md R18): every step such a cell takes
+//       the shifted equilibrium of the density and velocity of its upstream (x - 1) neighbour's stored DDFs
 // with load()/store() = the codecs of codecs.cpp applied at every read and write.
 // PARITY UNPINNED (no external pin exists; fixed by DESIGN.md section 3 only): the operation order of R5 / R10, the
 // pre-computation grouping of R7, rho_w = 1 in R9, writing both buffers in R11, R12 as the definition of the
@@ -108,13 +112,26 @@ T cdot(const int c[3], T vx, T vy, T vz) {
 // f = A (1/2 (B^2 + C) +- B) + D with A = w rho, B = 3 u.c_i, C = -3 u.u, D = w (rho - 1): 3 FMAs.
 // Surviving lines of equilibrium(): c3 = -3 (ux^2 + uy^2 + uz^2), rhom1 = rho - 1,
 // then u is multiplied by 3.
+// R17, shifted = false: eq (22), f = w rho ((u.c)^2 / (2 c^4) + u.c / c^2 + 1 - u.u / (2 c^2)), read with the
+// same A, B, C as eq (3): f = A ((1/2 (B^2 + C) +- B) + 1), the "+ 1" added last inside the bracket (grouping: DESIGN.md R17).
 template <class T>
-void equilibrium(const VelSet &vs, T rho, T ux, T uy, T uz, T *feq) {
+void equilibrium(const VelSet &vs, T rho, T ux, T uy, T uz, T *feq, bool shifted = true) {
     const T c3 = T(-3) * (ux * ux + uy * uy + uz * uz);
     const T rhom1 = rho - T(1);
     ux *= T(3);
     uy *= T(3);
     uz *= T(3);
+    if (!shifted) {
+        feq[0] = ((T)vs.w[0] * rho) * (T(0.5) * c3 + T(1));
+        for (int i = 1; i < vs.q; i += 2) {
+            const T A = (T)vs.w[i] * rho;
+            const T B = cdot<T>(vs.c[i], ux, uy, uz);
+            const T t = fma_t<T>(B, B, c3);
+            feq[i] = A * (fma_t<T>(T(0.5), t, B) + T(1));
+            feq[i + 1] = A * (fma_t<T>(T(0.5), t, -B) + T(1));
+        }
+        return;
+    }
     {
         const T w = (T)vs.w[0];
         feq[0] = fma_t<T>(w * rho, T(0.5) * c3, w * rhom1);
@@ -132,10 +149,10 @@ void equilibrium(const VelSet &vs, T rho, T ux, T uy, T uz, T *feq) {
 // R4: rho = f0 + f1 + ... + f(q-1), then + 1; momentum component a: pairs (i, i+1)
 // in index order, "+ (member with c_a = +1) - (the other)", strictly left to right.
 template <class T>
-void moments(const VelSet &vs, const T *f, T &rho, T j[3]) {
+void moments(const VelSet &vs, const T *f, T &rho, T j[3], bool shifted = true) {
     rho = f[0];
     for (int i = 1; i < vs.q; ++i) rho += f[i];
-    rho += T(1);
+    if (shifted) rho += T(1);                                  // eq (25); eq (20) without DDF-shifting
     for (int a = 0; a < 3; ++a) {
         bool first = true;
         T s = T(0);
@@ -155,6 +172,7 @@ void moments(const VelSet &vs, const T *f, T &rho, T j[3]) {
 struct orc_sim {
     int nx, ny, nz, fmt, arith;
     int collision;                    // ORC_BGK / ORC_TRT
+    bool shifted;                     // DDF-shifting (default); false: eqs (19)-(23), R17
     double lambda;                    // TRT magic parameter (R13)
     long N;
     VelSet vs;
@@ -205,7 +223,7 @@ void init_t(orc_sim *s, const T *rho, const T *u) {
 #pragma omp parallel for schedule(static)
     for (long n = 0; n < s->N; ++n) {
         T feq[27];
-        equilibrium<T>(vs, rho[n], u[n], u[s->N + n], u[2 * s->N + n], feq);
+        equilibrium<T>(vs, rho[n], u[n], u[s->N + n], u[2 * s->N + n], feq, s->shifted);
         for (int i = 0; i < vs.q; ++i) {
             store<T>(s, 0, i, n, feq[i]);
             store<T>(s, 1, i, n, feq[i]);
@@ -235,6 +253,19 @@ void step_t(orc_sim *s) {
                 const long n = x + (long)nx * (y + (long)ny * z);
                 if (s->flags[n] & (ORC_FLAG_WALL | ORC_FLAG_EQ)) continue;   // PAPER.md:1017; R15: E cells keep feq(rho0, u0)
                 T fh[27];
+                if (s->flags[n] & ORC_FLAG_OUT) {
+                    // R18: density and velocity of the upstream neighbour's stored DDFs (read-out rule R12: local moments,
+                    // u = (j - F/2) / rho, no clamp), imposed here as an equilibrium
+                    const long up = (x - 1 + nx) % nx + (long)nx * (y + (long)ny * z);
+                    for (int i = 0; i < q; ++i) fh[i] = load<T>(s, A, i, up);
+                    T rho, j[3], u[3];
+                    moments<T>(vs, fh, rho, j, s->shifted);
+                    for (int a = 0; a < 3; ++a) u[a] = (forced ? fma_t<T>(T(-0.5), F[a], j[a]) : j[a]) / rho;
+                    T feq[27];
+                    equilibrium<T>(vs, rho, u[0], u[1], u[2], feq, s->shifted);
+                    for (int i = 0; i < q; ++i) store<T>(s, Bb, i, n, feq[i]);
+                    continue;
+                }
                 fh[0] = load<T>(s, A, 0, n);
                 for (int i = 1; i < q; ++i) {
                     const int xs = (x - vs.c[i][0] + nx) % nx;        // R2, eq (24)
@@ -255,7 +286,7 @@ void step_t(orc_sim *s) {
                     }
                 }
                 T rho, j[3];
-                moments<T>(vs, fh, rho, j);                           // R4
+                moments<T>(vs, fh, rho, j, s->shifted);               // R4
                 T u[3];
                 for (int a = 0; a < 3; ++a) {                         // R5
                     const T ja = forced ? fma_t<T>(T(0.5), F[a], j[a]) : j[a];
@@ -263,7 +294,7 @@ void step_t(orc_sim *s) {
                     u[a] = std::fmin(std::fmax(u[a], -cs), cs);       // R6
                 }
                 T feq[27];
-                equilibrium<T>(vs, rho, u[0], u[1], u[2], feq);       // R7
+                equilibrium<T>(vs, rho, u[0], u[1], u[2], feq, s->shifted);   // R7
                 T uF = T(0);
                 if (forced) uF = u[0] * F[0] + u[1] * F[1] + u[2] * F[2];
                 if (s->collision == ORC_TRT) {
@@ -331,7 +362,7 @@ void read_t(orc_sim *s, T *rho_out, T *u_out) {
         }
         T fh[27], rho, j[3];
         for (int i = 0; i < vs.q; ++i) fh[i] = load<T>(s, s->cur, i, n);
-        moments<T>(vs, fh, rho, j);
+        moments<T>(vs, fh, rho, j, s->shifted);
         if (rho_out) rho_out[n] = rho;
         if (u_out)
             for (int a = 0; a < 3; ++a) {
@@ -377,6 +408,7 @@ orc_sim *orc_create(int nx, int ny, int nz, int velset, int fmt, int arith, doub
     s->cur = 0;
     s->steps_done = 0;
     s->collision = ORC_BGK;
+    s->shifted = true;
     s->lambda = 3.0 / 16.0;
     return s;
 }
@@ -385,6 +417,12 @@ int orc_set_collision(orc_sim *s, int collision, double lambda) {
     if (!s || (collision != ORC_BGK && collision != ORC_TRT) || !(lambda > 0.0)) return -1;
     s->collision = collision;
     s->lambda = s->arith == ORC_ARITH_F32 ? (double)(float)lambda : lambda;
+    return 0;
+}
+
+int orc_set_shifting(orc_sim *s, int on) {
+    if (!s) return -1;
+    s->shifted = on != 0;
     return 0;
 }
 

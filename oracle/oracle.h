@@ -23,7 +23,8 @@ enum { ORC_FP32 = 0, ORC_FP16S = 1, ORC_FP16C = 2, ORC_P16_0S = 3, ORC_P16_1S = 
        ORC_FP16 = 6, ORC_FP64 = 7 /* oracle only: raw doubles, needs arith = 1 */ };
 enum { ORC_ARITH_F32 = 0, ORC_ARITH_F64 = 1 };
 enum { ORC_BGK = 0, ORC_TRT = 1 /* textbook two-relaxation-time operator, NOT defined by the paper (R13) */ };
-enum { ORC_FLAG_WALL = 0x01, ORC_FLAG_EQ = 0x02 /* equilibrium boundary cell: keeps its init DDFs (R15) */ };
+enum { ORC_FLAG_WALL = 0x01, ORC_FLAG_EQ = 0x02 /* equilibrium boundary cell: keeps its init DDFs (R15) */,
+       ORC_FLAG_OUT = 0x04 /* zero-gradient outflow cell: equilibrium of its upstream (x - 1) neighbour's rho, u (R18) */ };
 
 /* ---- codecs (16-bit formats only, fmt in 1..6) ------------------------------------------------ */
 /* unscaled table value V(mag) of the 15-bit magnitude field, as a double (Inf/NaN for FP16 e=31) */
@@ -41,6 +42,8 @@ orc_sim *orc_create(int nx, int ny, int nz, int velset, int fmt, int arith, doub
 void orc_destroy(orc_sim *s);
 /* collision operator (default ORC_BGK) and, for ORC_TRT, the magic parameter Lambda (default 3/16); before orc_step */
 int  orc_set_collision(orc_sim *s, int collision, double lambda);
+/* DDF-shifting on (default) / off: off = eqs (19)-(23), the paper's negative control (R17); before orc_init */
+int  orc_set_shifting(orc_sim *s, int on);
 int  orc_set_flags(orc_sim *s, const uint8_t *flags);                 /* N bytes */
 int  orc_init(orc_sim *s, const float *rho, const float *u);         /* N, 3N (SoA) */
 int  orc_init_f64(orc_sim *s, const double *rho, const double *u);   /* arith = f64 only */

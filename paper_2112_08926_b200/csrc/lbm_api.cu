@@ -41,7 +41,7 @@ struct lbm {
     size_t scratch_bytes;
     long long steps;
     bool inited;
-    int V;                     // stream_collide variant in use: 1, 2, 4 cells per thread or LBM_VARIANT_BULK
+    int V;                     // stream_collide variant in use: 1, 2, 4 cells per thread or LBM_VARIANT_STAGED
     int V_request;             // LBM_VARIANT_AUTO = automatic
     const UnitOps *ops;
 };
@@ -147,8 +147,6 @@ int pick_variant(const lbm *h) {
     int want = h->V_request;
     const bool staged_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->staged_tile_cells() - 1) / h->ops->staged_tile_cells()) * h->ny * h->nz < 0x7FFFFFFFLL;
     if (want == LBM_VARIANT_STAGED && staged_ok) return LBM_VARIANT_STAGED;
-    const bool bulk_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->bulk_tile_cells() - 1) / h->ops->bulk_tile_cells()) * h->ny * h->nz <= 0x7FFFFFFFLL;
-    if (want == LBM_VARIANT_BULK && bulk_ok) return LBM_VARIANT_BULK;
     if (want == 0 && staged_ok && (h->fmt != LBM_FP32 || h->has_walls) && h->nx >= 64 && h->N >= (1LL << 20)) return LBM_VARIANT_STAGED;
     if (want != 1 && want != 2 && want != 4) want = (h->q == LBM_D2Q9 && h->fmt != LBM_FP32) ? 4 : 2;
     while (want > 1 && h->nx % want != 0) want >>= 1;
@@ -239,11 +237,12 @@ int lbm_bind(lbm_t *h, void *ddf_a, void *ddf_b, void *cuda_stream) {
 
 int lbm_set_variant(lbm_t *h, int v) {
     if (int rc = enter(h)) return rc;
-    if (v != LBM_VARIANT_AUTO && v != 1 && v != 2 && v != 4 && v != LBM_VARIANT_BULK && v != LBM_VARIANT_STAGED)
-        return fail(LBM_E_INVAL, "lbm_set_variant: 0 (auto), 1, 2, 4 (cells per thread), LBM_VARIANT_BULK or LBM_VARIANT_STAGED");
+    if (v == LBM_VARIANT_BULK) v = LBM_VARIANT_STAGED;           // the first staged kernel's name, kept for callers
+    if (v != LBM_VARIANT_AUTO && v != 1 && v != 2 && v != 4 && v != LBM_VARIANT_STAGED)
+        return fail(LBM_E_INVAL, "lbm_set_variant: 0 (auto), 1, 2, 4 (cells per thread) or LBM_VARIANT_STAGED");
     if ((v == 2 || v == 4) && h->nx % v != 0) return fail(LBM_E_INVAL, "lbm_set_variant: nx must be a multiple of the cells per thread");
-    const bool staged = v == LBM_VARIANT_BULK || v == LBM_VARIANT_STAGED;
-    if (staged && h->nx % 16 != 0) return fail(LBM_E_INVAL, "lbm_set_variant: the staged kernels need nx to be a multiple of 16");
+    const bool staged = v == LBM_VARIANT_STAGED;
+    if (staged && h->nx % 16 != 0) return fail(LBM_E_INVAL, "lbm_set_variant: the staged kernel needs nx to be a multiple of 16");
     if (staged && arith64(h->fmt)) return fail(LBM_E_UNSUPPORTED, "lbm_set_variant: the FP64-arithmetic formats have no staged kernel");
     drop_graphs(h);
     h->V_request = v;

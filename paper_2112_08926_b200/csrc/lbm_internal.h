@@ -9,17 +9,15 @@
 
 namespace lbmk {
 
-constexpr int VARIANT_BULK = 16;      // LBM_VARIANT_BULK of include/lbm.h
 constexpr int VARIANT_STAGED = 32;    // LBM_VARIANT_STAGED of include/lbm.h
 
 struct UnitOps {
-    // stream_collide: V = cells per thread (1, 2 or 4; nx % V == 0) of the per-thread kernel, or VARIANT_BULK
+    // stream_collide: V = cells per thread (1, 2 or 4; nx % V == 0) of the per-thread kernel, or VARIANT_STAGED
     // = the shared-memory-staged kernel (nx % 16 == 0); force = Guo term compiled in
     cudaError_t (*stream_collide)(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st);
     cudaError_t (*init)(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st);
     cudaError_t (*read)(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st);
     const char *(*name)(int V, int coll, bool force);
-    int (*bulk_tile_cells)();     // cells per tile of the staged kernel
     cudaError_t (*probe)(const void *A, const Params &p, bool force, const long long *cells, int count, float *rho, float *u,
                          cudaStream_t st);
     // FP64-arithmetic units only (lbm_unit64.cu), else null: read-out in double

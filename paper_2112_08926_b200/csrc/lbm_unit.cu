@@ -37,31 +37,6 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
 }
 
 
-// ---- the shared-memory-staged variant (lbm_bulk.cuh) ------------------------------------------------
-constexpr int BULK_NT = 256;
-
-BulkGeom bulk_geom(const Params &p, long long *tiles) {
-    typedef BulkShape<Q, F, BULK_NT> SH;
-    BulkGeom g;
-    g.tile_w = p.nx <= SH::RMAX * SH::TX ? p.nx : SH::RMAX * SH::TX;
-    g.tiles_per_row = (p.nx + g.tile_w - 1) / g.tile_w;
-    g.rows_per_tile = g.tiles_per_row == 1 ? SH::RMAX * SH::TX / p.nx : 1;
-    const int w_last = p.nx - (g.tiles_per_row - 1) * g.tile_w;
-    g.by_hw_full = FastDiv::make(g.tile_w / 2);
-    g.by_hw_last = FastDiv::make(w_last / 2);
-    g.ytiles = (p.ny + g.rows_per_tile - 1) / g.rows_per_tile;
-    *tiles = (long long)g.tiles_per_row * g.ytiles * p.nz;
-    g.n_tiles = (int)(*tiles < 0x7FFFFFFFLL ? *tiles : 0x7FFFFFFFLL);
-    g.by_tpr = FastDiv::make(g.tiles_per_row);
-    g.by_ytiles = FastDiv::make(g.ytiles);
-    for (int i = 0; i < 27; ++i) {
-        g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
-        g.src_boff[i] = g.dir_boff[i] = 0;                   // lbm_stage.cuh only
-    }
-    g.chunk_shift = 0;
-    return g;
-}
-
 // Resident CTAs of a persistent kernel on the CURRENT device (SMs x CTAs per SM), and the opt-in to its dynamic shared
 // memory.  Both are per-device state: resolved once per device and kernel, under a lock.  `cache` is the calling
 // launcher's own table (one per kernel instantiation).
@@ -88,27 +63,6 @@ cudaError_t resident_ctas(K kern, int threads, int smem, int *out, CtaCache &cac
     return cudaSuccess;
 }
 
-template <bool FORCE, int COLL = 0>
-cudaError_t launch_bulk(const void *A, void *B, const Params &p, cudaStream_t st) {
-    typedef BulkShape<Q, F, BULK_NT> SH;
-    auto kern = stream_collide_bulk_kernel<Q, F, BULK_NT, FORCE, COLL>;
-    int ctas = 0;
-    static CtaCache cache;                    // one per instantiation of this launcher
-    if (cudaError_t e = resident_ctas(kern, BULK_NT, SH::SMEM, &ctas, cache)) return e;
-    long long tiles = 0;
-    const BulkGeom g = bulk_geom(p, &tiles);
-    if (p.nx % 16 != 0 || tiles > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
-    const int grid = (int)(tiles < ctas ? tiles : ctas);
-    const EncEntry *tab = nullptr;
-    if (PairCodec<F>::TABLE) {
-        cudaError_t e = enc_table(F, &tab, st);
-        if (e != cudaSuccess) return e;
-    }
-    kern<<<grid, BULK_NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g, tab);
-    count_launch();
-    return cudaGetLastError();
-}
-
 // ---- the warp-specialised staged variant (lbm_stage.cuh) ----------------------------------------------
 BulkGeom stage_geom(const Params &p, long long *tiles) {
     typedef StageShape<Q, F> SH;
@@ -125,8 +79,7 @@ BulkGeom stage_geom(const Params &p, long long *tiles) {
     g.by_tpr = FastDiv::make(g.tiles_per_row);
     g.by_ytiles = FastDiv::make(g.ytiles);
     for (int i = 0; i < 27; ++i) {
-        g.src_off[i] = i < Q ? (long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2)) : 0;
-        g.src_boff[i] = g.src_off[i] * SH::ES;
+        g.src_boff[i] = i < Q ? ((long long)i * p.N - (long long)p.nx * (Lat<Q>::c(i, 1) + (long long)p.ny * Lat<Q>::c(i, 2))) * SH::ES : 0;
         g.dir_boff[i] = i < Q ? (long long)i * p.N * SH::ES : 0;
     }
     const int chunks_full = (g.rows_per_tile * (g.tile_w / 2) + 31) / 32;
@@ -171,12 +124,10 @@ cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int c
     }
     if (coll == 1) {
         // TRT (R13): the staged kernel, or the per-thread kernel with one, two or four cells per thread
-        if (V == VARIANT_BULK) return force ? launch_bulk<true, 1>(A, B, p, st) : launch_bulk<false, 1>(A, B, p, st);
         if (V == 4 && p.nx % 4 == 0) return force ? launch_sc<4, true, 1>(A, B, p, st) : launch_sc<4, false, 1>(A, B, p, st);
         if (V >= 2 && p.nx % 2 == 0) return force ? launch_sc<2, true, 1>(A, B, p, st) : launch_sc<2, false, 1>(A, B, p, st);
         return force ? launch_sc<1, true, 1>(A, B, p, st) : launch_sc<1, false, 1>(A, B, p, st);
     }
-    if (V == VARIANT_BULK) return force ? launch_bulk<true>(A, B, p, st) : launch_bulk<false>(A, B, p, st);
     switch (V * 2 + (force ? 1 : 0)) {
         case 2: return launch_sc<1, false>(A, B, p, st);
         case 3: return launch_sc<1, true>(A, B, p, st);
@@ -216,44 +167,27 @@ cudaError_t probe(const void *A, const Params &p, bool force, const long long *c
 }
 
 const char *name(int V, int coll, bool force) {
+#define LBM_KNAME(kernel, extra) kernel "<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) extra ">"
     if (V == VARIANT_STAGED) {
-        if (coll == 1)
-            return force ? "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
-                         : "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0,COLL=TRT>";
-        return force ? "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1>"
-                     : "stream_collide_staged_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0>";
+        if (coll == 1) return force ? LBM_KNAME("stream_collide_staged_kernel", ",FORCE=1,COLL=TRT") : LBM_KNAME("stream_collide_staged_kernel", ",FORCE=0,COLL=TRT");
+        return force ? LBM_KNAME("stream_collide_staged_kernel", ",FORCE=1") : LBM_KNAME("stream_collide_staged_kernel", ",FORCE=0");
     }
     if (coll == 1) {
-        if (V == VARIANT_BULK)
-            return force ? "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1,COLL=TRT>"
-                         : "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0,COLL=TRT>";
-        if (V == 4)
-            return force ? "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=1,COLL=TRT>"
-                         : "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=0,COLL=TRT>";
-        if (V >= 2)
-            return force ? "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=1,COLL=TRT>"
-                         : "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=0,COLL=TRT>";
-        return force ? "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=1,COLL=TRT>"
-                     : "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=0,COLL=TRT>";
+        if (V == 4) return force ? LBM_KNAME("stream_collide_kernel", ",V=4,FORCE=1,COLL=TRT") : LBM_KNAME("stream_collide_kernel", ",V=4,FORCE=0,COLL=TRT");
+        if (V >= 2) return force ? LBM_KNAME("stream_collide_kernel", ",V=2,FORCE=1,COLL=TRT") : LBM_KNAME("stream_collide_kernel", ",V=2,FORCE=0,COLL=TRT");
+        return force ? LBM_KNAME("stream_collide_kernel", ",V=1,FORCE=1,COLL=TRT") : LBM_KNAME("stream_collide_kernel", ",V=1,FORCE=0,COLL=TRT");
     }
-    static const char *names[4][2] = {
-        {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=0>",
-         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=1,FORCE=1>"},
-        {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=0>",
-         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=2,FORCE=1>"},
-        {"stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=0>",
-         "stream_collide_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",V=4,FORCE=1>"},
-        {"stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0>",
-         "stream_collide_bulk_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=1>"}};
-    return names[V == 1 ? 0 : V == 2 ? 1 : V == 4 ? 2 : 3][force ? 1 : 0];
+    if (V == 4) return force ? LBM_KNAME("stream_collide_kernel", ",V=4,FORCE=1") : LBM_KNAME("stream_collide_kernel", ",V=4,FORCE=0");
+    if (V == 2) return force ? LBM_KNAME("stream_collide_kernel", ",V=2,FORCE=1") : LBM_KNAME("stream_collide_kernel", ",V=2,FORCE=0");
+    return force ? LBM_KNAME("stream_collide_kernel", ",V=1,FORCE=1") : LBM_KNAME("stream_collide_kernel", ",V=1,FORCE=0");
+#undef LBM_KNAME
 }
 
-int bulk_tile_cells() { return 2 * BULK_NT; }
 int staged_tile_cells() { return StageShape<Q, F>::TC; }
 
 }  // namespace
 
 extern const UnitOps LBM_UNIT_SYMBOL;
-const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells, probe, nullptr, staged_tile_cells, build_fix_lists};
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, probe, nullptr, staged_tile_cells, build_fix_lists};
 
 }  // namespace lbmk

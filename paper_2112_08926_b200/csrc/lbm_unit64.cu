@@ -109,11 +109,10 @@ const char *name(int V, int coll, bool force) {
                  : "stream_collide64_kernel<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) ",FORCE=0>";
 }
 
-int bulk_tile_cells() { return 512; }   // unused: these units have no staged variant
 
 }  // namespace
 
 extern const UnitOps LBM_UNIT_SYMBOL;
-const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, bulk_tile_cells, probe, read64};
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, probe, read64};
 
 }  // namespace lbmk

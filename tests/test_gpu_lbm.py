@@ -146,7 +146,7 @@ def test_mass_conservation_fp32():
     assert abs(m1 - m0) / w.n_cells < 1e-6
 
 
-# ---- the shared-memory-staged kernel (lbm_bulk.cuh): same results, bit for bit ------------------------
+# ---- the shared-memory-staged kernel (lbm_stage.cuh): same results, bit for bit ------------------------
 # shapes: one tile per row (x wraps inside the segment), several tiles per row with a ragged last tile (halo
 # copies, wrap at the row ends), the smallest legal row (16 cells), 2-D
 BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16, 4, 5)), (19, (512, 2, 1)), (19, (1024, 3, 2)),
@@ -154,7 +154,7 @@ BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16
                (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1))]
 
 
-STAGED = [(lbm.VARIANT_BULK, "bulk"), (lbm.VARIANT_STAGED, "staged")]
+STAGED = [(lbm.VARIANT_STAGED, "staged")]
 
 
 @pytest.mark.parametrize("q,shape", BULK_SHAPES)
@@ -200,7 +200,7 @@ def test_automatic_variant_choice():
     assert "staged" in lbm.from_workload(w, "FP32").kernel_name
     w = wl.perturbed_equilibrium(36, 2, 2, seed=2)          # rows not 16-cell aligned: per-thread kernel
     assert "stream_collide_kernel" in lbm.from_workload(w, "FP16S").kernel_name
-    for v in (lbm.VARIANT_BULK, lbm.VARIANT_STAGED):
+    for v in (lbm.VARIANT_BULK, lbm.VARIANT_STAGED):        # (BULK: the staged kernel's first name, same kernel)
         with pytest.raises(lbm.LbmError):
             lbm.from_workload(w, "FP16S", variant=v)
 
@@ -267,7 +267,7 @@ def test_full_size_mass_conservation(full_size_workload):
 
 # ---- equilibrium boundary cells (LBM_FLAG_EQ, R15) and the Karman set-up of BASELINE configs[3] ----
 EQ_CASES = [(q, shape, v) for q, shape in [(19, (24, 9, 7)), (19, (272, 6, 5)), (27, (32, 7, 5)), (9, (48, 13, 1))]
-            for v in (1, 2, lbm.VARIANT_BULK, lbm.VARIANT_STAGED) if v < 16 or shape[0] % 16 == 0]
+            for v in (1, 2, lbm.VARIANT_STAGED) if v < 16 or shape[0] % 16 == 0]
 
 
 @pytest.mark.parametrize("q,shape,variant", EQ_CASES)

@@ -101,11 +101,11 @@ def test_trt_periodic_without_force(name):
     assert_parity(osim, gsim, name)
 
 
-# ---- staged kernels (lbm_bulk.cuh, lbm_stage.cuh): one tile per row, several tiles with a ragged last tile, D3Q27, D2Q9 -----
+# ---- staged kernel (lbm_stage.cuh): one tile per row, several tiles with a ragged last tile, D3Q27, D2Q9 -----
 @pytest.mark.parametrize("q,shape", [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 3, 2)), (27, (272, 3, 3)), (9, (1056, 3, 1))])
 @pytest.mark.parametrize("name", ALL_FORMATS)
 @pytest.mark.parametrize("walls", [False, True])
-@pytest.mark.parametrize("variant,tag", [(lbm.VARIANT_BULK, "bulk"), (lbm.VARIANT_STAGED, "staged")])
+@pytest.mark.parametrize("variant,tag", [(lbm.VARIANT_STAGED, "staged")])
 def test_trt_staged_kernel(q, shape, name, walls, variant, tag):
     w = wl.perturbed_equilibrium(*shape, seed=53, velset=q, tau=0.7)
     if walls:
@@ -125,7 +125,7 @@ def test_trt_lid_driven_cavity_small(name):
 
 
 @pytest.mark.parametrize("name", ["FP32", "FP16C"])
-@pytest.mark.parametrize("variant", [lbm.VARIANT_BULK, lbm.VARIANT_STAGED])
+@pytest.mark.parametrize("variant", [lbm.VARIANT_STAGED])
 def test_trt_equilibrium_boundary_cells(name, variant):
     w = wl.equilibrium_rim(wl.perturbed_equilibrium(48, 7, 5, seed=61, tau=0.65))
     osim, gsim = run_pair(w, name, 20, variant=variant)

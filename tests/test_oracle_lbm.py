@@ -239,6 +239,7 @@ def _reference_push_unshifted(w, steps):
     u = w.u.astype(np.float64).reshape((3,) + shape)
     wall = (w.flags.reshape(shape) & wl.FLAG_WALL) != 0
     eqb = (w.flags.reshape(shape) & wl.FLAG_EQ) != 0                 # equilibrium boundary cells (R15)
+    outb = (w.flags.reshape(shape) & wl.FLAG_OUT) != 0               # zero-gradient outflow cells (R18)
     F = np.array(w.force, np.float64)
     omega = 1.0 / w.tau
 
@@ -276,6 +277,11 @@ def _reference_push_unshifted(w, steps):
                 cF = c[i] @ F
                 uF = un[0] * F[0] + un[1] * F[1] + un[2] * F[2]
                 new[i] += (1 - 0.5 * omega) * wts[i] * (3 * (cF - uF) + 9 * cu * cF)
+        if outb.any():
+            # outflow cells: equilibrium of the upstream (x - 1) neighbour's state before this step
+            rho_up = np.roll(f.sum(0), 1, axis=2)
+            j_up = np.roll(np.einsum("ia,i...->a...", c.astype(np.float64), f), 1, axis=3)
+            new = np.where(outb[None], feq(rho_up, (j_up - 0.5 * F[:, None, None, None]) / rho_up), new)
         f = np.where(wall[None], f, new)                             # wall cells are never updated
         f = np.where(eqb[None], f_imposed, f)                        # E cells are reset to their imposed equilibrium
     rho_o = f.sum(0)
@@ -475,3 +481,99 @@ def test_trt_conserves_mass_and_momentum_and_keeps_the_viscosity(q, shape):
     amp = lambda u: (u[0] * w.u[0]).sum() / (w.u[0].astype(np.float64) ** 2).sum()
     rate = -math.log(amp(u200) / amp(u50)) / 150
     assert rate == pytest.approx(2 * (tau / 3 - 1 / 6) * (2 * math.pi / n) ** 2, rel=5e-3)
+
+
+# ---- R18: zero-gradient outflow cells (BASELINE configs[3]; not in the paper) ---------------------------------------
+@pytest.mark.parametrize("q,shape", [(19, (8, 6, 5)), (27, (7, 5, 4)), (9, (9, 7, 1))])
+def test_outflow_cells_against_push_reference(q, shape):
+    """walls, moving walls, an equilibrium inflow plane, an outflow plane and a body force together, vs the second
+    implementation (which imposes on an outflow cell the equilibrium of its upstream neighbour's previous state)"""
+    w = wl.perturbed_equilibrium(*shape, seed=17, velset=q, rho_sigma=1e-2, tau=0.8)
+    w = wl.random_walls(w, 0.1, seed=8, moving_fraction=0.5)
+    f = w.flags.reshape(w.nz, w.ny, w.nx).copy()
+    f[:, :, 0] = wl.FLAG_EQ
+    f[:, :, -1] = wl.FLAG_OUT
+    w.flags = f.reshape(-1)
+    w.force = (1e-4, -2e-4, 0.0 if q == 9 else 3e-4)
+    s = sim64(w)
+    s.step(9)
+    rho, u = s.read_rho_u(f64=True)
+    rref, uref = _reference_push_unshifted(w, 9)
+    assert np.abs(rho - rref).max() < 5e-14
+    assert np.abs(u - uref).max() < 5e-14
+
+
+def test_outflow_keeps_uniform_flow_and_has_zero_gradient():
+    """Inflow by equilibrium cells at x = 0, outflow cells at x = nx-1, periodic in y and z.  (i) A uniform state is a
+    fixed point.  (ii) Started at rest, the channel starts to flow, and at the outflow plane density and velocity equal
+    the upstream neighbour's of the step before (that is the definition), so the gradient there vanishes as the flow
+    becomes steady."""
+    ue = (0.05, 0.0, 0.0)
+
+    def box(u_init):
+        w = wl.perturbed_equilibrium(24, 5, 3, seed=1, rho_sigma=0.0, u_abs_max=0.0, tau=0.8)
+        f = w.flags.reshape(w.nz, w.ny, w.nx).copy()
+        f[:, :, 0] = wl.FLAG_EQ
+        f[:, :, -1] = wl.FLAG_OUT
+        w.flags = f.reshape(-1)
+        u = np.zeros((3, w.nz, w.ny, w.nx), np.float32)
+        u[0] = u_init
+        u[0, :, :, 0] = ue[0]
+        w.u = u.reshape(3, -1)
+        return w
+    w = box(ue[0])
+    s = sim64(w)
+    s.step(50)
+    rho, u = s.read_rho_u(f64=True)
+    assert np.abs(rho - 1.0).max() < 1e-13 and np.abs(u[0] - np.float32(ue[0])).max() < 1e-13 and np.abs(u[1:]).max() < 1e-14
+    w = box(0.0)
+    s = sim64(w)
+    s.step(1999)
+    rho_a, u_a = s.read_rho_u(f64=True)
+    s.step(1)
+    rho_b, u_b = s.read_rho_u(f64=True)
+    ux_a, ux_b = u_a[0].reshape(w.nz, w.ny, w.nx), u_b[0].reshape(w.nz, w.ny, w.nx)
+    assert np.abs(ux_b[:, :, -1] - ux_a[:, :, -2]).max() < 1e-15          # the definition, one step apart
+    assert np.abs(rho_b.reshape(w.nz, w.ny, w.nx)[:, :, -1] - rho_a.reshape(w.nz, w.ny, w.nx)[:, :, -2]).max() < 1e-15
+    assert ux_b[:, :, 1:].min() > 0.2 * ue[0]                              # the channel flows downstream, out through the plane
+    assert np.abs(ux_b[:, :, -1] - ux_b[:, :, -2]).max() < 1e-6            # zero gradient at the outflow
+
+
+# ---- R17: without DDF-shifting, eqs (19)-(23) (PAPER.md:651-667): the paper's negative control -------------------------
+@pytest.mark.parametrize("q,shape,force", [(19, (6, 5, 4), (1e-4, -2e-4, 3e-4)), (27, (4, 5, 4), (0.0, 0.0, 0.0)), (9, (7, 6, 1), (1e-4, 2e-4, 0.0))])
+def test_unshifted_variant(q, shape, force):
+    """In FP64 the unshifted step equals the second implementation (itself unshifted, plain eq (22)) and the shifted
+    step to rounding, and what it stores is the shifted DDF plus the lattice weight."""
+    w = wl.perturbed_equilibrium(*shape, seed=19, velset=q, rho_sigma=1e-2, tau=0.7)
+    w = wl.random_walls(w, 0.15, seed=5, moving_fraction=0.5)
+    w.force = force
+    a = oracle.from_workload(w, oracle.FP64, oracle.ARITH_F64, shifted=False)
+    b = sim64(w)
+    a.step(7)
+    b.step(7)
+    rho, u = a.read_rho_u(f64=True)
+    rref, uref = _reference_push_unshifted(w, 7)
+    assert np.abs(rho - rref).max() < 5e-14 and np.abs(u - uref).max() < 5e-14
+    rho_s, u_s = b.read_rho_u(f64=True)
+    assert np.abs(rho - rho_s).max() < 5e-14 and np.abs(u - u_s).max() < 5e-14
+    _, wts, _ = oracle.velocity_set(q)
+    fluid = w.flags == 0
+    for i in range(q):
+        assert np.abs(a.read_ddf(i)[fluid] - b.read_ddf(i)[fluid] - wts[i]).max() < 5e-15
+
+
+def test_shifting_is_what_makes_16_bit_storage_accurate():
+    """PAPER.md:314-316 (Fig. 8, dashed curves): without DDF-shifting the 16-bit formats lose the Taylor-Green decay;
+    with it they follow the FP64 run.  2-D Taylor-Green, D2Q9, FP16C and FP16S storage, FP32 arithmetic."""
+    w = wl.taylor_green_2d(32, 32, 1)
+    ref = sim64(w)
+    ref.step(100)
+    _, uref = ref.read_rho_u(f64=True)
+    for fmt in (oracle.FP16C, oracle.FP16S, oracle.P16_1S):
+        err = {}
+        for shifted in (True, False):
+            s = oracle.from_workload(w, fmt, shifted=shifted)
+            s.step(100)
+            _, u = s.read_rho_u()
+            err[shifted] = np.abs(u - uref).max() / np.abs(uref).max()
+        assert err[True] < 0.02 and err[False] > 5 * err[True], (fmt, err)

@@ -21,6 +21,7 @@ import numpy as np
 
 FLAG_WALL = 0x01
 FLAG_EQ = 0x02      # equilibrium boundary cell (TYPE_E)
+FLAG_OUT = 0x04     # zero-gradient outflow cell (BASELINE configs[3]; R18)
 
 # velocity-set / collision / storage-format ids of include/lbm.h (interface constants, not arithmetic)
 D2Q9, D3Q19, D3Q27 = 9, 19, 27
@@ -163,12 +164,14 @@ def random_walls(w: Workload, fraction: float, seed: int = 7, moving_fraction: f
 
 
 def karman_vortex_street(nx: int = 256, ny: int = 64, nz: int = 16, radius: float = 4.0, x_cyl: int | None = None,
-                         u_in: float = 0.05, tau: float | None = None, Re: float = 200.0, velset: int = D3Q19) -> Workload:
+                         u_in: float = 0.05, tau: float | None = None, Re: float = 200.0, velset: int = D3Q19,
+                         outflow: bool = False) -> Workload:
     """BASELINE.json configs[3] (shape of PAPER.md:320-336): a channel with a z-spanning cylinder of wall cells at
     (x_cyl, ny/2), flow along +x.  The x = 0, x = nx-1, y = 0 and y = ny-1 planes are equilibrium boundary cells
     holding rho = 1, u = (u_in, 0, 0) (the paper enforces the velocity on the box perimeter with equilibrium
     boundaries); z is periodic.  Asymmetric start as in PAPER.md:330: the fluid moves with u_in in
     one half of the box (y < ny/2) and rests in the other, so that shedding starts at once in every number format.
+    outflow=True replaces the equilibrium cells of the x = nx-1 plane by zero-gradient outflow cells (BASELINE's wording).
     tau defaults to the value Re = 2 R u_in / nu gives."""
     if x_cyl is None:
         x_cyl = nx // 4
@@ -182,6 +185,8 @@ def karman_vortex_street(nx: int = 256, ny: int = 64, nz: int = 16, radius: floa
     flags[(x - x_cyl) ** 2 + (y - ny // 2) ** 2 <= radius * radius] = FLAG_WALL
     rim = (x == 0) | (x == nx - 1) | (y == 0) | (y == ny - 1)
     flags[rim] = FLAG_EQ
+    if outflow:                                    # BASELINE's "zero-gradient outflow": the x = nx-1 plane between the y rims
+        flags[(x == nx - 1) & (y > 0) & (y < ny - 1)] = FLAG_OUT
     ux = np.where(rim | (y < ny // 2), u_in, 0.0)
     ux[flags == FLAG_WALL] = 0.0
     u = _pack(ux.reshape(-1), np.zeros(N), np.zeros(N))
