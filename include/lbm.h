@@ -60,8 +60,13 @@ enum {
  * LBM_FLAG_EQ:   equilibrium boundary cell (TYPE_E; "equilibrium boundaries"; R15): it keeps
  *                the DDFs lbm_init gave it -- the shifted equilibrium of its rho, u -- for ever; its neighbours pull
  *                from it as from a fluid cell (inflow / outflow / free-stream perimeter).
- * Neither kind of cell is written by lbm_step; lbm_read_rho_u returns for them the fields given to lbm_init. */
-enum { LBM_FLAG_WALL = 0x01, LBM_FLAG_EQ = 0x02 };
+ * Neither kind of cell is written by lbm_step; lbm_read_rho_u returns for them the fields given to lbm_init.
+ * LBM_FLAG_OUT:  zero-gradient outflow cell (BASELINE configs[3] "zero-gradient outflow"; NOT in the paper: DESIGN.md R18):
+ *                every step it takes the shifted equilibrium of the density and velocity of its upstream neighbour, the
+ *                cell at x - 1 (periodic), as that neighbour's stored DDFs give them (local moments, u = (j - F/2) / rho).
+ *                Neighbours pull from it as from a fluid cell; lbm_read_rho_u reads it like a fluid cell.
+ * A cell carries at most one of the three bits. */
+enum { LBM_FLAG_WALL = 0x01, LBM_FLAG_EQ = 0x02, LBM_FLAG_OUT = 0x04 };
 enum {
     LBM_OK = 0,
     LBM_E_INVAL = -1,       /* bad argument                                   */
@@ -102,7 +107,13 @@ int lbm_set_cells_per_thread(lbm_t *h, int v);
  * called at any time between steps; takes effect from the next lbm_step. */
 int lbm_set_trt_lambda(lbm_t *h, double lambda);
 
-/* Set the cell flags.  flags: HOST pointer, N bytes, copied.  Only LBM_FLAG_WALL or LBM_FLAG_EQ may be set (not both on one cell)
+/* The paper's negative control (eqs (19)-(23); dashed curves of PAPER.md:265, 316): on = 0 stores f_i
+ * instead of f_i - w_i, sums rho without the "+1" and takes f^eq from eq (22) (R17).  Default on = 1.  Before
+ * lbm_init (else LBM_E_STATE); not for the FP64-arithmetic formats (LBM_E_UNSUPPORTED).  The control runs on the
+ * per-thread kernel with one cell per thread: it exists to show what DDF-shifting buys, not to be fast. */
+int lbm_set_shifting(lbm_t *h, int on);
+
+/* Set the cell flags.  flags: HOST pointer, N bytes, copied.  One of LBM_FLAG_WALL, LBM_FLAG_EQ, LBM_FLAG_OUT per cell, or none
  * (else LBM_E_INVAL).  Must precede lbm_init (LBM_E_STATE otherwise).  Synchronises the stream. */
 int lbm_set_flags(lbm_t *h, const unsigned char *flags);
 
@@ -112,6 +123,14 @@ int lbm_set_flags(lbm_t *h, const unsigned char *flags);
  * lbm_init_device takes DEVICE pointers read asynchronously on the handle's stream. */
 int lbm_init(lbm_t *h, const float *rho, const float *u);
 int lbm_init_device(lbm_t *h, const float *rho_dev, const float *u_dev);
+/* The same with the fields of BASELINE configs[4] drawn cell by cell from a counter-based generator instead of read from
+ * memory ("random-perturbed equilibrium init (rho = 1 + N(0, 1e-3), |u| <= 0.05 from seed)"): for boxes whose input
+ * fields (16 bytes per cell) do not fit beside the DDFs -- the largest cubes of the bandwidth sweep.  The recipe
+ * (splitmix64 of seed and cell index; rho = 1 + sqrt(3) 1e-3 (a0 + a1 + a2 + a3 - 2), u = (2 a - 1) 0.05 / sqrt(3), a_k
+ * 22-bit uniforms) is stated in csrc/lbm_kernels.cuh and typed a second time, in numpy, in workloads.generated_fields.
+ * Boxes without flagged cells only (LBM_E_STATE); not for the FP64-arithmetic formats (LBM_E_UNSUPPORTED).
+ * Asynchronous on the handle's stream. */
+int lbm_init_generated(lbm_t *h, unsigned long long seed);
 
 /* Advance n >= 0 time steps: n launches of the fused stream-collide kernel (Listing 2,
  * PAPER.md:1014-1042; eqs (24)-(28)), alternating the two buffers.

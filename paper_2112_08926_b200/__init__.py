@@ -28,7 +28,7 @@ BGK, TRT = 0, 1
 FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C": 5, "FP16": 6,
            "FP64": 7, "FP64_FP32": 8}     # 7, 8: FP64 arithmetic with double / float storage
 FORMAT_NAMES = {v: k for k, v in FORMATS.items()}
-FLAG_WALL, FLAG_EQ = 0x01, 0x02
+FLAG_WALL, FLAG_EQ, FLAG_OUT = 0x01, 0x02, 0x04
 VARIANT_AUTO, VARIANT_BULK, VARIANT_STAGED = 0, 16, 32
 OK, E_INVAL, E_UNSUPPORTED, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 
@@ -43,8 +43,10 @@ SYMBOLS = {
     "lbm_set_flags": (_i, [_p, _p]),
     "lbm_init": (_i, [_p, _p, _p]),
     "lbm_init_device": (_i, [_p, _p, _p]),
+    "lbm_init_generated": (_i, [_p, C.c_ulonglong]),
     "lbm_step": (_i, [_p, _i]),
     "lbm_set_graphs": (_i, [_p, _i]),
+    "lbm_set_shifting": (_i, [_p, _i]),
     "lbm_read_rho_u": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_device": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_f64": (_i, [_p, _p, _p]),
@@ -128,7 +130,7 @@ class Simulation:
     """One LBM box on the current CUDA device.  Mirrors the C ABI call for call."""
 
     def __init__(self, nx, ny, nz, velset=D3Q19, ddf_format="FP32", tau=0.6, force=None, collision=BGK,
-                 use_torch_memory=True, cells_per_thread=0, variant=0):
+                 use_torch_memory=True, cells_per_thread=0, variant=0, shifted=True):
         self._h = C.c_void_p()
         self.nx, self.ny, self.nz, self.q = int(nx), int(ny), int(nz), int(velset)
         self.N = self.nx * self.ny * self.nz
@@ -153,6 +155,8 @@ class Simulation:
             _check(lib().lbm_set_cells_per_thread(self._h, int(cells_per_thread)))
         if variant:
             _check(lib().lbm_set_variant(self._h, int(variant)))
+        if not shifted:
+            _check(lib().lbm_set_shifting(self._h, 0))
 
     # -- lifetime ------------------------------------------------------------------------------
     def close(self):
@@ -206,8 +210,15 @@ class Simulation:
             raise ValueError("rho must have N and u 3N entries")
         _check(lib().lbm_init(self._h, _np_ptr(rho), _np_ptr(u)))
 
+    def init_generated(self, seed: int):
+        """fields drawn on the device, cell by cell (workloads.generated_fields gives the same values on the host)"""
+        _check(lib().lbm_init_generated(self._h, int(seed)))
+
     def step(self, n: int = 1):
         _check(lib().lbm_step(self._h, int(n)))
+
+    def set_shifting(self, on: bool):
+        _check(lib().lbm_set_shifting(self._h, 1 if on else 0))
 
     def set_graphs(self, enable: bool):
         _check(lib().lbm_set_graphs(self._h, 1 if enable else 0))

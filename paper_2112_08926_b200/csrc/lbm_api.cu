@@ -37,6 +37,7 @@ struct lbm {
     uint2 *fix_cells; // first use after lbm_set_flags, only when the box has flagged cells
     cudaGraphExec_t gexec[2];  // lbm_step on small boxes: GRAPH_STEPS launches captured once, starting from buffer 0 / 1
     bool graphs;               // lbm_set_graphs
+    bool shifted;              // lbm_set_shifting (default true)
     void *scratch;             // device staging area of the host-pointer calls (lbm_init, lbm_read_rho_u*), kept between calls
     size_t scratch_bytes;
     long long steps;
@@ -88,6 +89,7 @@ Params make_params(const lbm *h) {
     p.tau = h->tau;
     p.fix_off = h->fix_off;
     p.fix_cells = h->fix_cells;
+    p.shifted = h->shifted ? 1 : 0;
     return p;
 }
 
@@ -143,7 +145,7 @@ int ensure_ddf(lbm *h) {
 //   * everything else (ragged rows, small L2-resident / launch-bound boxes): the per-thread kernel, 4 cells per thread
 //     for D2Q9 16-bit, else 2.
 int pick_variant(const lbm *h) {
-    if (arith64(h->fmt)) return 1;
+    if (arith64(h->fmt) || !h->shifted) return 1;            // (the unshifted control: one kernel, one cell per thread)
     int want = h->V_request;
     const bool staged_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->staged_tile_cells() - 1) / h->ops->staged_tile_cells()) * h->ny * h->nz < 0x7FFFFFFFLL;
     if (want == LBM_VARIANT_STAGED && staged_ok) return LBM_VARIANT_STAGED;
@@ -197,6 +199,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, int velset, int collision, i
     h->omega = 1.0f / tau;
     h->trt_lambda = 3.0 / 16.0;
     h->graphs = true;
+    h->shifted = true;
     for (int a = 0; a < 3; ++a) {
         h->force[a] = force ? force[a] : 0.0f;
         if (h->force[a] != 0.0f) h->has_force = true;
@@ -272,8 +275,8 @@ int lbm_set_flags(lbm_t *h, const unsigned char *flags) {
     if (h->inited) return fail(LBM_E_STATE, "lbm_set_flags: must be called before lbm_init");
     bool walls = false;
     for (long long n = 0; n < h->N; ++n) {
-        if (flags[n] & ~(LBM_FLAG_WALL | LBM_FLAG_EQ)) return fail(LBM_E_INVAL, "lbm_set_flags: unknown flag bit set");
-        if (flags[n] == (LBM_FLAG_WALL | LBM_FLAG_EQ)) return fail(LBM_E_INVAL, "lbm_set_flags: a cell cannot be wall and equilibrium boundary");
+        if (flags[n] & ~(LBM_FLAG_WALL | LBM_FLAG_EQ | LBM_FLAG_OUT)) return fail(LBM_E_INVAL, "lbm_set_flags: unknown flag bit set");
+        if (flags[n] & (flags[n] - 1)) return fail(LBM_E_INVAL, "lbm_set_flags: a cell is a wall, an equilibrium boundary or an outflow cell, not several");
         walls |= flags[n] != 0;
     }
     h->has_walls = walls;
@@ -311,7 +314,7 @@ static int init_from_device(lbm *h, const float *rho_dev, const float *u_dev) {
         u = h->u0;
         LBM_CUDA_TRY(lbmk::launch_mark_moving(h->q, h->bounce, h->u0, h->nx, h->ny, h->nz, h->stream));
     }
-    LBM_CUDA_TRY(h->ops->init(h->ddf[0], h->ddf[1], r, u, h->N, h->stream));
+    LBM_CUDA_TRY(h->ops->init(h->ddf[0], h->ddf[1], r, u, h->N, h->shifted, h->stream));
     h->cur = 0;
     h->steps = 0;
     h->inited = true;
@@ -323,6 +326,21 @@ int lbm_init_device(lbm_t *h, const float *rho_dev, const float *u_dev) {
     if (int rc = enter(h)) return rc;
     if (!rho_dev || !u_dev) return fail(LBM_E_INVAL, "lbm_init_device: rho and u must not be NULL");
     return init_from_device(h, rho_dev, u_dev);
+}
+
+int lbm_init_generated(lbm_t *h, unsigned long long seed) {
+    if (int rc = enter(h)) return rc;
+    if (arith64(h->fmt) || !h->ops->init_generated) return fail(LBM_E_UNSUPPORTED, "lbm_init_generated: not for the FP64-arithmetic formats");
+    if (h->has_walls) return fail(LBM_E_STATE, "lbm_init_generated: the box has flagged cells (their fields must be given: lbm_init)");
+    if (!h->shifted) return fail(LBM_E_UNSUPPORTED, "lbm_init_generated: with DDF-shifting only");
+    if (int rc = ensure_ddf(h)) return rc;
+    drop_graphs(h);
+    LBM_CUDA_TRY(h->ops->init_generated(h->ddf[0], h->ddf[1], h->N, seed, h->stream));
+    h->cur = 0;
+    h->steps = 0;
+    h->inited = true;
+    h->V = pick_variant(h);
+    return LBM_OK;
 }
 
 int lbm_init(lbm_t *h, const float *rho, const float *u) {
@@ -401,6 +419,15 @@ int lbm_step(lbm_t *h, int n) {
         }
     }
     return step_plain(h, p, n);
+}
+
+int lbm_set_shifting(lbm_t *h, int on) {
+    if (int rc = enter(h)) return rc;
+    if (h->inited) return fail(LBM_E_STATE, "lbm_set_shifting: must be called before lbm_init");
+    if (!on && arith64(h->fmt)) return fail(LBM_E_UNSUPPORTED, "lbm_set_shifting: the FP64-arithmetic formats run with DDF-shifting only");
+    h->shifted = on != 0;
+    drop_graphs(h);
+    return LBM_OK;
 }
 
 int lbm_set_graphs(lbm_t *h, int enable) {

@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(256) mark_near_kernel(const unsigned char *__r
     const int y = blockIdx.y, z = blockIdx.z;
     if (x >= nx) return;
     const long long n = x + (long long)nx * (y + (long long)ny * z);
-    unsigned fl = in[n] & FLAG_FIXED;
+    unsigned fl = in[n] & (FLAG_FIXED | FLAG_OUT);          // (an outflow cell pulls nothing: no FLAG_NEAR for it)
     unsigned mask = 0;                                       // bit i: the pull source of direction i is a wall cell
     if (!fl) {
         unsigned near = 0;

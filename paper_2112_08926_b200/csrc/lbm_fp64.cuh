@@ -196,6 +196,28 @@ stream_collide64_kernel(const S *__restrict__ A, S *__restrict__ B, const Params
     if (flag & FLAG_FIXED) return;                                       // PAPER.md:1017; R15
 
     double f[Q];
+    if (flag & FLAG_OUT) {
+        // R18 (not in the paper): zero-gradient outflow cell -- the equilibrium of the upstream (x - 1) neighbour's density
+        // and velocity (read-out rule R12: local moments of its stored DDFs, u = (j - F/2) / rho, no clamp)
+        const S *Ai = A + own + dxv[0];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            f[i] = ld(Ai);
+            Ai += p.N;
+        }
+        double rho, j[3], u[3];
+        moments<Q>(f, rho, j);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) u[a] = __ddiv_rn(FORCE ? fma_(-0.5, d.F[a], j[a]) : j[a], rho);
+        equilibrium<Q>(rho, u[0], u[1], u[2], f);
+        S *Bo = B + own;
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            st(Bo, f[i]);
+            Bo += p.N;
+        }
+        return;
+    }
     if (!(flag & FLAG_NEAR)) {
         const S *Ai = A + own;
 #pragma unroll

@@ -15,7 +15,7 @@ struct UnitOps {
     // stream_collide: V = cells per thread (1, 2 or 4; nx % V == 0) of the per-thread kernel, or VARIANT_STAGED
     // = the shared-memory-staged kernel (nx % 16 == 0); force = Guo term compiled in
     cudaError_t (*stream_collide)(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st);
-    cudaError_t (*init)(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st);
+    cudaError_t (*init)(void *A, void *B, const float *rho, const float *u, long long N, bool shifted, cudaStream_t st);
     cudaError_t (*read)(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st);
     const char *(*name)(int V, int coll, bool force);
     cudaError_t (*probe)(const void *A, const Params &p, bool force, const long long *cells, int count, float *rho, float *u,
@@ -26,6 +26,8 @@ struct UnitOps {
     // builder of the per-tile flagged-pair lists (Params::fix_off / fix_cells; the caller cudaFrees both)
     int (*staged_tile_cells)();
     cudaError_t (*build_fix_lists)(const Params &p, unsigned **off, uint2 **list, cudaStream_t st);
+    // init from the counter-based generator of lbm_kernels.cuh (null in the FP64-arithmetic units)
+    cudaError_t (*init_generated)(void *A, void *B, long long N, unsigned long long seed, cudaStream_t st);
 };
 
 const UnitOps *unit_ops(int q, int fmt);   // lbm_units.cu (table of all compiled units)

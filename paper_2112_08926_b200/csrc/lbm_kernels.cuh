@@ -163,10 +163,29 @@ struct PullDirWall<Q, F, Q> {
                                                float (&)[Q]) {}
 };
 
+// R18 (not in the paper): a zero-gradient outflow cell n takes the equilibrium of the density and velocity of
+// its upstream neighbour's stored DDFs (read-out rule R12: local moments, u = (j - F/2) / rho, no clamp)
+template <int Q, int F, bool FORCE, bool SHIFT = true>
+__device__ __forceinline__ void outflow_cell(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B,
+                                             const Params &p, long long n, long long n_up) {
+    typedef Elem<F> E;
+    float f[Q], rho, j[3], u[3];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i] = E::ld1(A + (long long)i * p.N + n_up);
+    moments<Q, SHIFT>(f, rho, j);
+    const float Fv[3] = {p.fx, p.fy, p.fz};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) u[a] = __fdiv_rn(FORCE ? fma_(-0.5f, Fv[a], j[a]) : j[a], rho);
+    float feq[Q];
+    equilibrium<Q, SHIFT>(rho, u[0], u[1], u[2], feq);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + n, feq[i]);
+}
+
 constexpr int SC_THREADS = 256;
 
 // grid: x = tiles of BX*V cells along x, y = tiles of BY rows, z = plane.  blockDim = (BX, BY), BX*BY = SC_THREADS
-template <int Q, int F, int V, bool FORCE, int COLL = 0>
+template <int Q, int F, int V, bool FORCE, int COLL = 0, bool SHIFT = true>
 __global__ void __launch_bounds__(SC_THREADS)
 stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params p) {
     typedef Elem<F> E;
@@ -201,7 +220,7 @@ stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F
         // ---- fast path: a3 load + decode, a5-a9 collide, a10 encode + store, all vectorised --------
         PullDir<Q, F, V, 0>::run(A, p.N, rows, x0, xm, xp, f);
 #pragma unroll
-        for (int j = 0; j < V; ++j) collide<COLL, Q, FORCE>(f[j], p);
+        for (int j = 0; j < V; ++j) collide<COLL, Q, FORCE, 0, 0, SHIFT>(f[j], p);
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             float o[V];
@@ -218,9 +237,13 @@ stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F
             if ((any >> (8 * j)) & FLAG_FIXED) continue;                   // PAPER.md:1017; R15
             const int x = x0 + j;
             const int xmj = x == 0 ? p.nx - 1 : x - 1, xpj = x == p.nx - 1 ? 0 : x + 1;
+            if ((any >> (8 * j)) & FLAG_OUT) {                             // R18
+                outflow_cell<Q, F, FORCE, SHIFT>(A, B, p, own + j, rows[1][1] + xmj);
+                continue;
+            }
             float g[Q];
             PullDirWall<Q, F, 0>::run(A, p, rows, x, xmj, xpj, g);
-            collide<COLL, Q, FORCE>(g, p);
+            collide<COLL, Q, FORCE, 0, 0, SHIFT>(g, p);
 #pragma unroll
             for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + own + j, g[i]);
         }
@@ -228,14 +251,58 @@ stream_collide_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F
 }
 
 // ---- init: every cell, walls included, both buffers (R11) -----------------------
-template <int Q, int F>
+template <int Q, int F, bool SHIFT = true>
 __global__ void __launch_bounds__(256)
 init_kernel(typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const float *__restrict__ rho,
             const float *__restrict__ u, long long N) {
     typedef Elem<F> E;
     for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
         float feq[Q];
-        equilibrium<Q>(__ldg(rho + n), __ldg(u + n), __ldg(u + N + n), __ldg(u + 2 * N + n), feq);
+        equilibrium<Q, SHIFT>(__ldg(rho + n), __ldg(u + n), __ldg(u + N + n), __ldg(u + 2 * N + n), feq);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            unsigned w[1];
+            const float o[1] = {feq[i]};
+            E::template pack<1>(w, o);
+            Raw<E::SIZE>::st(A + (long long)i * N + n, w);
+            Raw<E::SIZE>::st(B + (long long)i * N + n, w);
+        }
+    }
+}
+
+// ---- init from a counter-based generator (BASELINE configs[4]: "random-perturbed equilibrium init (rho = 1 + N(0, 1e-3),
+// |u| <= 0.05 from seed)") -------------------------------------------------------------------
+// For the largest cubes the input fields (16 bytes per cell) do not fit beside the DDFs, so the cell draws them itself:
+//   z(k)  = splitmix64(seed + (8 n + k) * 0x9E3779B97F4A7C15), k = 0..6;   a_k = (z(k) >> 42) * 2^-22  in [0, 1)
+//   rho   = 1 + ((a_0 + a_1) + (a_2 + a_3) - 2) * 1.7320508e-3f      (sum of four uniforms: variance 1/3, times sqrt(3) 1e-3)
+//   u_a   = (2 a_{4+a} - 1) * 0.028867513f                            (0.05 / sqrt(3): |u| <= 0.05)
+// every operation an IEEE FP32 one on exactly representable operands, so that workloads.generated_fields (numpy, typed
+// on its own) yields the same bits for the oracle.  D2Q9: u_z = 0.
+__device__ __forceinline__ unsigned long long splitmix64(unsigned long long z) {
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27; z *= 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    return z;
+}
+__device__ __forceinline__ void generated_fields(unsigned long long seed, long long n, bool two_d, float &rho, float (&u)[3]) {
+    float a[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k)
+        a[k] = (float)(unsigned)(splitmix64(seed + (8ull * (unsigned long long)n + k) * 0x9E3779B97F4A7C15ull) >> 42) * 2.384185791015625e-07f;
+    const float g = sub(add(add(a[0], a[1]), add(a[2], a[3])), 2.0f);
+    rho = add(1.0f, mul(g, 1.7320508e-3f));
+#pragma unroll
+    for (int k = 0; k < 3; ++k) u[k] = mul(sub(mul(2.0f, a[4 + k]), 1.0f), 0.028867513f);
+    if (two_d) u[2] = 0.0f;
+}
+template <int Q, int F>
+__global__ void __launch_bounds__(256)
+init_generated_kernel(typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, long long N, unsigned long long seed) {
+    typedef Elem<F> E;
+    for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
+        float rho, u[3], feq[Q];
+        generated_fields(seed, n, Q == 9, rho, u);
+        equilibrium<Q>(rho, u[0], u[1], u[2], feq);
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             unsigned w[1];
@@ -248,7 +315,7 @@ init_kernel(typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict
 }
 
 // ---- read-out: local moments of the current buffer (R12) -------------------------------------------
-template <int Q, int F, bool FORCE>
+template <int Q, int F, bool FORCE, bool SHIFT = true>
 __global__ void __launch_bounds__(256)
 read_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, float *__restrict__ rho_out,
                   float *__restrict__ u_out) {
@@ -264,7 +331,7 @@ read_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, flo
             float f[Q];
 #pragma unroll
             for (int i = 0; i < Q; ++i) f[i] = E::ld1(A + (long long)i * N + n);
-            moments<Q>(f, rho, j);
+            moments<Q, SHIFT>(f, rho, j);
             const float Fv[3] = {p.fx, p.fy, p.fz};
 #pragma unroll
             for (int a = 0; a < 3; ++a) u[a] = __fdiv_rn(FORCE ? fma_(-0.5f, Fv[a], j[a]) : j[a], rho);
@@ -278,7 +345,7 @@ read_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, flo
 }
 
 // ---- read-out at selected cells (R12), for probes in long runs ---------------------------------------
-template <int Q, int F, bool FORCE>
+template <int Q, int F, bool FORCE, bool SHIFT = true>
 __global__ void __launch_bounds__(128)
 probe_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, const long long *__restrict__ cells, int count,
                    float *__restrict__ rho_out, float *__restrict__ u_out) {
@@ -295,7 +362,7 @@ probe_rho_u_kernel(const typename Elem<F>::T *__restrict__ A, const Params p, co
         float f[Q];
 #pragma unroll
         for (int i = 0; i < Q; ++i) f[i] = E::ld1(A + (long long)i * N + n);
-        moments<Q>(f, rho, j);
+        moments<Q, SHIFT>(f, rho, j);
         const float Fv[3] = {p.fx, p.fy, p.fz};
 #pragma unroll
         for (int a = 0; a < 3; ++a) u[a] = __fdiv_rn(FORCE ? fma_(-0.5f, Fv[a], j[a]) : j[a], rho);

@@ -291,6 +291,10 @@ __device__ __forceinline__ void fix_cell(const typename Elem<F>::T *__restrict__
         for (int i = 0; i < Q; ++i) B[(long long)i * p.N + n] = __ldg(A + (long long)i * p.N + n);
         return;
     }
+    if (fl & FLAG_OUT) {                                                     // R18: zero-gradient outflow cell
+        outflow_cell<Q, F, FORCE>(A, B, p, n, n - x + (x == 0 ? p.nx - 1 : x - 1));
+        return;
+    }
     const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
     const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
     const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};

@@ -23,7 +23,7 @@ namespace {
 constexpr int Q = LBM_Q, F = LBM_F;
 typedef typename Elem<F>::T T;
 
-template <int V, bool FORCE, int COLL = 0>
+template <int V, bool FORCE, int COLL = 0, bool SHIFT = true>
 cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) {
     const int tx = (p.nx + V - 1) / V;
     int bx = 1;
@@ -31,7 +31,7 @@ cudaError_t launch_sc(const void *A, void *B, const Params &p, cudaStream_t st) 
     const int by = SC_THREADS / bx;
     const dim3 block(bx, by, 1);
     const dim3 grid((tx + bx - 1) / bx, (p.ny + by - 1) / by, p.nz);
-    stream_collide_kernel<Q, F, V, FORCE, COLL><<<grid, block, 0, st>>>((const T *)A, (T *)B, p);
+    stream_collide_kernel<Q, F, V, FORCE, COLL, SHIFT><<<grid, block, 0, st>>>((const T *)A, (T *)B, p);
     count_launch();
     return cudaGetLastError();
 }
@@ -118,6 +118,11 @@ cudaError_t build_fix_lists(const Params &p, unsigned **off_out, uint2 **list_ou
 }
 
 cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
+    if (!p.shifted) {
+        // R17, the paper's negative control (eqs (19)-(23)): the per-thread kernel, one cell per thread
+        if (coll == 1) return force ? launch_sc<1, true, 1, false>(A, B, p, st) : launch_sc<1, false, 1, false>(A, B, p, st);
+        return force ? launch_sc<1, true, 0, false>(A, B, p, st) : launch_sc<1, false, 0, false>(A, B, p, st);
+    }
     if (V == VARIANT_STAGED) {
         if (coll == 1) return force ? launch_staged<true, 1>(A, B, p, st) : launch_staged<false, 1>(A, B, p, st);
         return force ? launch_staged<true>(A, B, p, st) : launch_staged<false>(A, B, p, st);
@@ -145,14 +150,24 @@ int blocks_for(long long N) {
     return (int)(b < cap ? (b < 1 ? 1 : b) : cap);
 }
 
-cudaError_t init(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st) {
-    init_kernel<Q, F><<<blocks_for(N), 256, 0, st>>>((T *)A, (T *)B, rho, u, N);
+cudaError_t init(void *A, void *B, const float *rho, const float *u, long long N, bool shifted, cudaStream_t st) {
+    if (shifted) init_kernel<Q, F, true><<<blocks_for(N), 256, 0, st>>>((T *)A, (T *)B, rho, u, N);
+    else init_kernel<Q, F, false><<<blocks_for(N), 256, 0, st>>>((T *)A, (T *)B, rho, u, N);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t init_generated(void *A, void *B, long long N, unsigned long long seed, cudaStream_t st) {
+    init_generated_kernel<Q, F><<<blocks_for(N), 256, 0, st>>>((T *)A, (T *)B, N, seed);
     count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t read(const void *A, const Params &p, bool force, float *rho, float *u, cudaStream_t st) {
-    if (force) read_rho_u_kernel<Q, F, true><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
+    if (!p.shifted) {
+        if (force) read_rho_u_kernel<Q, F, true, false><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
+        else read_rho_u_kernel<Q, F, false, false><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
+    } else if (force) read_rho_u_kernel<Q, F, true><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
     else read_rho_u_kernel<Q, F, false><<<blocks_for(p.N), 256, 0, st>>>((const T *)A, p, rho, u);
     count_launch();
     return cudaGetLastError();
@@ -160,13 +175,17 @@ cudaError_t read(const void *A, const Params &p, bool force, float *rho, float *
 
 cudaError_t probe(const void *A, const Params &p, bool force, const long long *cells, int count, float *rho, float *u, cudaStream_t st) {
     const int blocks = (count + 127) / 128;
-    if (force) probe_rho_u_kernel<Q, F, true><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
+    if (!p.shifted) {
+        if (force) probe_rho_u_kernel<Q, F, true, false><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
+        else probe_rho_u_kernel<Q, F, false, false><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
+    } else if (force) probe_rho_u_kernel<Q, F, true><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
     else probe_rho_u_kernel<Q, F, false><<<blocks, 128, 0, st>>>((const T *)A, p, cells, count, rho, u);
     count_launch();
     return cudaGetLastError();
 }
 
 const char *name(int V, int coll, bool force) {
+    // (the unshifted control, Params::shifted == 0, always runs stream_collide_kernel<V=1,...,SHIFT=0>)
 #define LBM_KNAME(kernel, extra) kernel "<Q=" LBM_STR(LBM_Q) ",F=" LBM_STR(LBM_F) extra ">"
     if (V == VARIANT_STAGED) {
         if (coll == 1) return force ? LBM_KNAME("stream_collide_staged_kernel", ",FORCE=1,COLL=TRT") : LBM_KNAME("stream_collide_staged_kernel", ",FORCE=0,COLL=TRT");
@@ -188,6 +207,6 @@ int staged_tile_cells() { return StageShape<Q, F>::TC; }
 }  // namespace
 
 extern const UnitOps LBM_UNIT_SYMBOL;
-const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, probe, nullptr, staged_tile_cells, build_fix_lists};
+const UnitOps LBM_UNIT_SYMBOL = {stream_collide, init, read, name, probe, nullptr, staged_tile_cells, build_fix_lists, init_generated};
 
 }  // namespace lbmk

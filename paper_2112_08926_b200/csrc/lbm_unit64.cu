@@ -68,7 +68,7 @@ int blocks_for(long long N) {
     return (int)(b < cap ? (b < 1 ? 1 : b) : cap);
 }
 
-cudaError_t init(void *A, void *B, const float *rho, const float *u, long long N, cudaStream_t st) {
+cudaError_t init(void *A, void *B, const float *rho, const float *u, long long N, bool /*shifted: always*/, cudaStream_t st) {
     init64_kernel<Q, S><<<blocks_for(N), 256, 0, st>>>((S *)A, (S *)B, rho, u, N);
     count_launch();
     return cudaGetLastError();

@@ -29,7 +29,7 @@ def test_call_order_and_flags_validation():
         s.step(1)
     assert e.value.code == lbm.E_STATE
     with pytest.raises(lbm.LbmError) as e:
-        s.set_flags(np.full(128, 4, np.uint8))
+        s.set_flags(np.full(128, 8, np.uint8))
     assert e.value.code == lbm.E_INVAL
     s.init(np.ones(128, np.float32), np.zeros((3, 128), np.float32))
     with pytest.raises(lbm.LbmError) as e:

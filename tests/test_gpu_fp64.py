@@ -101,6 +101,21 @@ def test_equilibrium_rim(name):
     assert_parity(osim, gsim, name)
 
 
+@pytest.mark.parametrize("q,shape", [(19, (24, 9, 7)), (27, (12, 8, 6))])
+@pytest.mark.parametrize("name", list(F64_FORMATS))
+def test_outflow_cells(q, shape, name):
+    """zero-gradient outflow cells (LBM_FLAG_OUT, R18) with an equilibrium inflow plane, walls and a force"""
+    w = wl.perturbed_equilibrium(*shape, seed=41, velset=q, tau=0.75)
+    w = wl.random_walls(w, 0.08, seed=43, moving_fraction=0.5)
+    f = w.flags.reshape(w.nz, w.ny, w.nx).copy()
+    f[:, :, 0] = lbm.FLAG_EQ
+    f[:, :, -1] = lbm.FLAG_OUT
+    w.flags = f.reshape(-1)
+    w.force = (1e-5, 0.0, 0.0)
+    osim, gsim = run_pair(w, name, 20)
+    assert_parity(osim, gsim, name)
+
+
 def test_all_cells_walls_is_a_noop():
     w = wl.perturbed_equilibrium(8, 4, 4, seed=1)
     w.flags[:] = wl.FLAG_WALL

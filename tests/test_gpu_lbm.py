@@ -20,9 +20,9 @@ ALL_FORMATS = list(FORMATS)
 TOL = {name: (1e-6 if name == "FP32" else 1e-3) for name in ALL_FORMATS}
 
 
-def run_pair(w, name, steps, cells_per_thread=0, variant=0):
-    osim = oracle.from_workload(w, FORMATS[name])
-    gsim = lbm.from_workload(w, name, cells_per_thread=cells_per_thread, variant=variant)
+def run_pair(w, name, steps, cells_per_thread=0, variant=0, shifted=True):
+    osim = oracle.from_workload(w, FORMATS[name], shifted=shifted)
+    gsim = lbm.from_workload(w, name, cells_per_thread=cells_per_thread, variant=variant, shifted=shifted)
     osim.step(steps)
     gsim.step(steps)
     return osim, gsim
@@ -300,14 +300,137 @@ def test_karman_config4_small(name):
     assert np.abs(ou[1]).max() > 1e-4            # the wake is not symmetric: shedding has started
 
 
+# ---- zero-gradient outflow cells (LBM_FLAG_OUT, R18) ---------------------------------------------------
+OUT_CASES = [(q, shape, v) for q, shape in [(19, (24, 9, 7)), (19, (272, 6, 5)), (27, (32, 7, 5)), (9, (48, 13, 1))]
+             for v in (1, 2, lbm.VARIANT_STAGED) if v < 16 or shape[0] % 16 == 0]
+
+
+def _with_inflow_and_outflow(w):
+    f = w.flags.reshape(w.nz, w.ny, w.nx).copy()
+    f[:, :, 0] = lbm.FLAG_EQ
+    f[:, :, -1] = lbm.FLAG_OUT
+    f[:, 2, 5:9] = lbm.FLAG_OUT            # (and a few in the interior, next to walls and fluid)
+    w.flags = f.reshape(-1)
+    return w
+
+
+@pytest.mark.parametrize("q,shape,variant", OUT_CASES)
+@pytest.mark.parametrize("name", ALL_FORMATS)
+def test_outflow_cells(q, shape, name, variant):
+    w = wl.perturbed_equilibrium(*shape, seed=41, velset=q, tau=0.75)
+    w = wl.random_walls(w, 0.08, seed=43, moving_fraction=0.5)
+    w = _with_inflow_and_outflow(w)
+    w.force = (1e-5, 0.0, 0.0)
+    osim, gsim = run_pair(w, name, 20, variant=variant)
+    assert_parity(osim, gsim, name)
+
+
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "P16_2C"])
+def test_karman_with_outflow_plane_small(name):
+    """configs[3] as BASELINE words it (equilibrium inflow, zero-gradient outflow) at oracle size"""
+    w = wl.karman_vortex_street(128, 48, 8, radius=3.0, u_in=0.05, outflow=True)
+    assert (w.flags == lbm.FLAG_OUT).sum() == 46 * 8
+    osim, gsim = run_pair(w, name, 400)
+    assert_parity(osim, gsim, name)
+
+
+# ---- without DDF-shifting (eqs (19)-(23), PAPER.md:651-667; DESIGN.md R17): the paper's negative control -----------------
+@pytest.mark.parametrize("q,shape", [(19, (24, 9, 7)), (27, (16, 6, 5)), (9, (33, 9, 1))])
+@pytest.mark.parametrize("name", ALL_FORMATS)
+def test_unshifted_control(q, shape, name):
+    w = wl.perturbed_equilibrium(*shape, seed=47, velset=q, tau=0.7)
+    w = wl.random_walls(w, 0.08, seed=49, moving_fraction=0.5)
+    w = _with_inflow_and_outflow(w)
+    w.force = (1e-5, -2e-5, 0.0 if q == 9 else 3e-5)
+    osim, gsim = run_pair(w, name, 15, shifted=False)
+    assert "V=1" in gsim.kernel_name
+    assert_parity(osim, gsim, name)
+    osim2 = oracle.from_workload(w, FORMATS[name], shifted=False)
+    osim2.set_collision(oracle.TRT)
+    gsim2 = lbm.from_workload(w, name, shifted=False, collision=lbm.TRT)      # TRT too
+    osim2.step(9)
+    gsim2.step(9)
+    assert_parity(osim2, gsim2, name)
+
+
+def test_unshifted_control_api():
+    s = lbm.Simulation(8, 4, 4, 19, "FP64", 0.6)
+    with pytest.raises(lbm.LbmError) as e:
+        s.set_shifting(False)
+    assert e.value.code == lbm.E_UNSUPPORTED
+    w = wl.taylor_green_3d(16)
+    g = lbm.from_workload(w, "FP16C")
+    with pytest.raises(lbm.LbmError) as e:
+        g.set_shifting(False)                                   # after init
+    assert e.value.code == lbm.E_STATE
+
+
 def test_flag_validation_with_equilibrium_bit():
     s = lbm.Simulation(8, 4, 4, 19, "FP32", 0.6)
     fl = np.zeros(128, np.uint8)
     fl[3] = lbm.FLAG_WALL | lbm.FLAG_EQ
     with pytest.raises(lbm.LbmError):
         s.set_flags(fl)
-    fl[3] = 4
+    fl[3] = 8
     with pytest.raises(lbm.LbmError):
         s.set_flags(fl)
+    fl[3] = lbm.FLAG_OUT | lbm.FLAG_WALL
+    with pytest.raises(lbm.LbmError):
+        s.set_flags(fl)
+    fl[3] = lbm.FLAG_OUT
+    s.set_flags(fl)
     fl[3] = lbm.FLAG_EQ
     s.set_flags(fl)
+
+
+# ---- fields drawn on the device (lbm_init_generated) and boxes beyond 2^31 cells ---------------------------------------
+@pytest.mark.parametrize("q,shape", [(19, (48, 7, 5)), (27, (16, 6, 5)), (9, (64, 9, 1))])
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "P16_1S"])
+def test_generated_init_equals_the_host_recipe(q, shape, name):
+    """The device draws rho, u cell by cell (splitmix64 of seed and cell index); workloads.generated_fields restates the
+    recipe in numpy: the oracle initialised with those arrays must hold the same DDF codes, before and after steps."""
+    n = shape[0] * shape[1] * shape[2]
+    rho, u = wl.generated_fields(np.arange(n), 20211208, two_d=(q == 9))
+    w = wl.Workload("generated", *shape, q, 0.6, rho, u, np.zeros(n, np.uint8))
+    o = oracle.from_workload(w, FORMATS[name])
+    g = lbm.Simulation(*shape, q, name, 0.6)
+    g.init_generated(20211208)
+    for steps in (0, 5):
+        o.step(steps)
+        g.step(steps)
+        for i in range(q):
+            assert np.array_equal(g.read_ddf(i), o.read_ddf(i)), (name, i, steps)
+    g.close()
+
+
+def test_more_than_2_to_31_cells():
+    """Cell indices beyond 2^31 (the paper's 32-bit index stops at 608^3; BASELINE configs[4]'s largest
+    16-bit cube, 1312^3, has 2.26e9 cells): a D2Q9 FP16S box of 65536 x 33024 = 2.164e9 cells (80 GB), drawn on the
+    device, three steps; sampled blocks -- some across the periodic faces, some in the last rows, whose indices need 32
+    bits -- are stepped by the oracle from the same recipe and must agree bit for bit at the probed cells."""
+    import torch
+    torch.cuda.empty_cache()
+    nx, ny, steps, blk = 65536, 33024, 3, 14
+    assert nx * ny > 2 ** 31
+    g = lbm.Simulation(nx, ny, 1, 9, "FP16S", 0.6)
+    g.init_generated(7)
+    g.step(steps)
+    assert "staged" in g.kernel_name
+    rng = np.random.default_rng(3)
+    origins = [(-7, -7), (nx - 7, ny - 7), (12345, ny - blk), (nx - blk, 40000 % ny)]
+    origins += [(int(rng.integers(0, nx)), int(rng.integers(0, ny))) for _ in range(8)]
+    c = slice(3, blk - 3)
+    for ox, oy in origins:
+        xs, ys = np.arange(ox, ox + blk) % nx, np.arange(oy, oy + blk) % ny
+        cells = (xs[None, :] + nx * ys[:, None].astype(np.int64)).reshape(-1)
+        rho, u = wl.generated_fields(cells, 7, two_d=True)
+        sub = wl.Workload("block", blk, blk, 1, 9, 0.6, rho, u, np.zeros(blk * blk, np.uint8))
+        o = oracle.from_workload(sub, FORMATS["FP16S"])
+        o.step(steps)
+        orho, ou = o.read_rho_u()
+        core = cells.reshape(blk, blk)[c, c].reshape(-1)
+        grho, gu = g.read_rho_u_at(core)
+        assert np.array_equal(grho.view(np.uint32), orho.reshape(blk, blk)[c, c].reshape(-1).view(np.uint32)), (ox, oy)
+        assert np.array_equal(gu.view(np.uint32), ou.reshape(3, blk, blk)[:, c, c].reshape(3, -1).view(np.uint32)), (ox, oy)
+    g.close()
+    torch.cuda.empty_cache()

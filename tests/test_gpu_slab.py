@@ -34,7 +34,10 @@ def test_slabs_equal_the_whole_box(q, shape, parts, name):
     steps = 9
     s = _run(w, name, parts, steps)
     if name == "FP64":
-        o = oracle.from_workload(w, oracle.FP64, oracle.ARITH_F64)
+        # (the C ABI takes tau and the force as floats: the FP64 oracle gets them rounded the same way, R16)
+        import dataclasses
+        w64 = dataclasses.replace(w, tau=float(np.float32(w.tau)), force=tuple(float(np.float32(v)) for v in w.force))
+        o = oracle.from_workload(w64, oracle.FP64, oracle.ARITH_F64)
     else:
         o = oracle.from_workload(w, FORMATS[name])
     o.step(steps)

@@ -224,3 +224,30 @@ def codec_probe_inputs(seed: int = 1, per_binade: int = 4096) -> np.ndarray:
     special = np.array([0.0, -0.0, np.inf, -np.inf, np.nan, 1.0, -1.0, 2.0, -2.0, 65504.0, 65520.0,
                         3.4e38, 1e-45, 1.1754944e-38], np.float32)
     return np.concatenate([x, -x, special])
+
+
+def generated_fields(cells, seed: int, two_d: bool = False):
+    """rho [k], u [3, k] (float32) of the cells with indices `cells` as the library's lbm_init_generated draws them on
+    the device (include/lbm.h; the recipe is restated here, not shared): for cell n and k = 0..6
+        z = splitmix64(seed + (8 n + k) * 0x9E3779B97F4A7C15),   a_k = (z >> 42) * 2^-22   in [0, 1)
+        rho = 1 + ((a_0 + a_1) + (a_2 + a_3) - 2) * float32(1.7320508e-3)       (all float32, IEEE)
+        u_a = (2 a_{4+a} - 1) * float32(0.028867513);   u_z = 0 for D2Q9.
+    Inputs only: boxes too large for host arrays (BASELINE configs[4]'s largest cubes) are checked on sampled blocks."""
+    n = np.asarray(cells, dtype=np.uint64).reshape(-1)
+    mask = np.uint64(0xFFFFFFFFFFFFFFFF)
+    a = []
+    with np.errstate(over="ignore"):
+        for k in range(7):
+            z = (np.uint64(seed & 0xFFFFFFFFFFFFFFFF) + (np.uint64(8) * n + np.uint64(k)) * np.uint64(0x9E3779B97F4A7C15)) & mask
+            z ^= z >> np.uint64(30)
+            z = (z * np.uint64(0xBF58476D1CE4E5B9)) & mask
+            z ^= z >> np.uint64(27)
+            z = (z * np.uint64(0x94D049BB133111EB)) & mask
+            z ^= z >> np.uint64(31)
+            a.append(((z >> np.uint64(42)).astype(np.float32)) * np.float32(2.0 ** -22))
+    g = ((a[0] + a[1]) + (a[2] + a[3])) - np.float32(2.0)
+    rho = np.float32(1.0) + g * np.float32(1.7320508e-3)
+    u = np.stack([(np.float32(2.0) * a[4 + k] - np.float32(1.0)) * np.float32(0.028867513) for k in range(3)])
+    if two_d:
+        u[2] = 0.0
+    return rho.astype(np.float32), u.astype(np.float32)
