@@ -434,3 +434,56 @@ def test_more_than_2_to_31_cells():
         assert np.array_equal(gu.view(np.uint32), ou.reshape(3, blk, blk)[:, c, c].reshape(3, -1).view(np.uint32)), (ox, oy)
     g.close()
     torch.cuda.empty_cache()
+
+
+# ---- BASELINE config 3 at its real size: 128^3 cavity on the staged kernel, sampled blocks WITH the wall shell and the lid -----
+# Information does not cross a wall cell (a pull from a wall is a bounce), so a block whose face lies in the wall shell
+# needs no margin on that side: the oracle steps the block as a periodic box of its own and, away from the block's
+# interior-side faces (>= `steps` + 1 cells), every cell -- walls, cells next to walls, cells under the moving lid -- must
+# agree with the 128^3 GPU run bit for bit.
+CAV_L, CAV_STEPS, CAV_BLK = 128, 4, 16
+
+
+def _cavity_blocks(L, blk):
+    hi = L - blk
+    return [(0, 0, 0), (hi, hi, hi), (0, 40, hi), (56, 0, 60), (hi, 70, 0), (30, hi, hi), (50, 60, hi), (48, 52, 44)]
+
+
+@pytest.mark.parametrize("collision", ["BGK", "TRT"])
+@pytest.mark.parametrize("name", ["FP32", "FP16S", "FP16C", "P16_1S"])
+def test_cavity_config3_full_size_sampled_blocks(name, collision):
+    L, blk, m = CAV_L, CAV_BLK, CAV_STEPS + 1
+    w = wl.lid_driven_cavity(L)
+    g = lbm.from_workload(w, name, collision=lbm.TRT if collision == "TRT" else lbm.BGK)
+    assert "staged" in g.kernel_name
+    g.step(CAV_STEPS)
+    grho, gu = g.read_rho_u()
+    gd = [g.read_ddf(i).reshape(L, L, L) for i in range(19)]
+    g.close()
+    grho, gu = grho.reshape(L, L, L), gu.reshape(3, L, L, L)
+    fl3, rho3, u3 = w.flags.reshape(L, L, L), w.rho.reshape(L, L, L), w.u.reshape(3, L, L, L)
+    for ox, oy, oz in _cavity_blocks(L, blk):
+        sl = (slice(oz, oz + blk), slice(oy, oy + blk), slice(ox, ox + blk))
+        sub = wl.Workload("block", blk, blk, blk, 19, w.tau, np.ascontiguousarray(rho3[sl]).reshape(-1),
+                          np.ascontiguousarray(u3[(slice(None),) + sl]).reshape(3, -1), np.ascontiguousarray(fl3[sl]).reshape(-1))
+        o = oracle.from_workload(sub, FORMATS[name])
+        if collision == "TRT":
+            o.set_collision(oracle.TRT)
+        o.step(CAV_STEPS)
+        orho, ou = o.read_rho_u()
+        # margin on the sides where the block ends inside the fluid, none where it ends in the wall shell
+        core = tuple(slice(0 if o0 == 0 else m, blk if o0 + blk == L else blk - m) for o0 in (oz, oy, ox))
+        assert np.array_equal(grho[sl][core].view(np.uint32), orho.reshape(blk, blk, blk)[core].view(np.uint32)), (name, ox, oy, oz)
+        assert np.array_equal(gu[(slice(None),) + sl][(slice(None),) + core].view(np.uint32),
+                              ou.reshape(3, blk, blk, blk)[(slice(None),) + core].view(np.uint32)), (name, ox, oy, oz)
+        for i in range(19):
+            assert np.array_equal(gd[i][sl][core], o.read_ddf(i).reshape(blk, blk, blk)[core]), (name, i, ox, oy, oz)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name", ["FP32", "FP16S"])
+def test_lid_driven_cavity_config3_copy_full_length(name):
+    """config 3's oracle-sized copy (32^3, same tau and lid velocity) for the full scaled step count, 12 500"""
+    w = wl.lid_driven_cavity(32, tau=0.5384)
+    osim, gsim = run_pair(w, name, 12500)
+    assert_parity(osim, gsim, name)
