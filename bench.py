@@ -18,8 +18,10 @@ body force, default 256) and configs[3] (Karman street 4L x L x L/4 with a cylin
 L = 256, i.e. 1024 x 256 x 64), inputs from workloads/: same JSON line, same roofline accounting (2 q s + 1 bytes per
 cell), clocks and cpu_baseline.
 
-N > 1 (torchrun): the path does not exchange data between GPUs in this tier:
-every rank runs an independent replica of the box ("weak" scaling), timed as the max over ranks.
+N > 1 (torchrun): by default every rank runs an independent replica of the box ("weak" scaling, no data-path
+collective: the paper's path is one GPU), timed as the max over ranks.  --decomposition slab
+instead runs ONE box L x L x (L n_gpus) cut into z-slabs with the halo exchange of paper_2112_08926_b200/slab.py after
+every step; with one GPU it runs the same plan as two slabs on that device.
 """
 from __future__ import annotations
 
@@ -322,6 +324,109 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slab(args):
+    """--decomposition slab: ONE periodic box L x L x (L * n_gpus), cut
+    into z slabs, one per rank, every step followed by the exchange of the face-crossing directions in the stored
+    format (paper_2112_08926_b200/slab.py; NCCL point-to-point).  Weak scaling: L^3 owned cells per GPU.  With one
+    GPU the same plan runs as two half-height slabs of an L^3 box on that device (device copies instead of NCCL): the
+    cost of the ghost planes and of the copies, not a multi-GPU number."""
+    import torch
+
+    import paper_2112_08926_b200 as lbm
+    from paper_2112_08926_b200 import slab as sl
+
+    world, rank, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    K, W, Q = args.steps, args.warmup, args.velset
+    if Q == 9 or args.workload != "periodic":
+        raise SystemExit("--decomposition slab: the periodic D3Q19 / D3Q27 box only")
+    L = args.size if args.size else 512
+    formats = [f for f in args.formats.split(",") if not f.startswith("FP64")]
+    peak, peak_src = measured_peak()
+    coll = lbm.TRT if args.collision == "TRT" else lbm.BGK
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    windows, results, launches_total = [], {}, 0
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for name in formats:
+        if world > 1:
+            box = sl.DistSlab(L, L, L * world, Q, name, TAU, collision=coll)
+            slabs = [box.slab]
+        else:
+            box = sl.LocalSlabs(L, L, L, 2, Q, name, TAU, collision=coll)
+            slabs = box.slabs
+        for k, s in enumerate(slabs):                         # owned planes drawn on the device, ghosts by one exchange
+            s.sim.init_generated(rank_seed(rank) + 1000 * k)
+        if world > 1:
+            sl.exchange_distributed(box.slab.current(), box.slab.plan, rank, world, dist)
+        else:
+            box.exchange()
+        box.step(W)
+        barrier()
+        n0 = lbm.launch_count()
+        t0 = sampler.mark()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        box.step(K)                                           # K x (stream_collide on every local slab + exchange)
+        e1.record()
+        barrier()
+        windows.append((t0, sampler.mark()))
+        ms = max_over_ranks(e0.elapsed_time(e1))
+        launches = lbm.launch_count() - n0
+        launches_total += launches
+        prho, _ = slabs[0].sim.read_rho_u_at(np.linspace(0, slabs[0].sim.N - 1, 4096).astype(np.int64))
+        assert bool(np.isfinite(prho).all()), name
+        owned = L ** 3                                        # per GPU
+        computed = sum(s.sim.N for s in slabs)          # ghost planes included
+        bpc = lbm.bytes_per_cell(Q, name)
+        up, down = sl.crossing_directions(Q)
+        halo = (len(up) + len(down)) * L * L * slabs[0].es * len(slabs)
+        gbs = computed * bpc / (ms / K * 1e-3) / 1e9
+        results[name] = {"mlups": round(world * owned * K / (ms * 1e-3) / 1e6, 1), "ms_per_step": round(ms / K, 4),
+                         "bytes_per_cell": bpc, "hbm_gbs": round(gbs, 1), "frac_of_peak": round(gbs / peak, 4),
+                         "halo_bytes_sent_per_gpu_per_step": halo, "kernel": slabs[0].sim.kernel_name, "launches": launches}
+        box.close()
+        del box, slabs
+        torch.cuda.empty_cache()
+    sampler.stop()
+    if rank != 0:
+        return
+    head = HEADLINE if HEADLINE in results else formats[0]
+    r = results[head]
+    line = {
+        "metric": METRIC, "value": r["mlups"], "unit": "MLUPs/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": (f"ONE periodic D3Q{Q} box {L}x{L}x{L * world} in {world} z-slabs of {L} planes + 2 ghost planes, "
+                                f"one per GPU, halo exchange (NCCL point-to-point) every step" if world > 1 else
+                                f"periodic D3Q{Q} box {L}^3 as two z-slabs of {L // 2} planes + 2 ghost planes on ONE GPU, "
+                                "halo exchange by device copies every step (the decomposition's overhead, not a multi-GPU number)")
+                               + f"; perturbed equilibrium drawn on the device, tau {TAU}; {args.collision}; headline storage format {head}",
+                   "cells": L ** 3 * world, "l2_policy": "inputs larger than L2" if L >= 256 else "partly L2-resident",
+                   "parallelism": f"z-slab decomposition over {world} GPU(s)"},
+        "formats": results,
+        "roofline": {"bound": "hbm", "kernel": r["kernel"], "achieved": r["hbm_gbs"], "peak": peak, "unit": "GB/s",
+                     "frac": r["frac_of_peak"], "traffic": None, "peak_source": peak_src,
+                     "what": "per GPU; counts the ghost planes' cells (computed, then overwritten) and the whole step incl. the exchange"},
+        "e2e": {"value": None, "unit": "MLUPs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                "what": "no end-to-end leg in this mode (input drawn on the device); see the default run"},
+        "gpu_launches": launches_total, "clocks": sampler.summary(windows),
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def cpu_model():
     try:
         for line in open("/proc/cpuinfo"):
@@ -403,12 +508,16 @@ def main():
     ap.add_argument("--device-init", action="store_true", help="draw the input on the device (big sweep sizes)")
     ap.add_argument("--cells-per-thread", type=int, default=0, help="0 = library default")
     ap.add_argument("--collision", default="BGK", choices=["BGK", "TRT"], help="sweep only; the headline is BGK (TRT: DESIGN.md R13)")
+    ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent boxes (default) or ONE box cut into z-slabs with a halo exchange per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomposition == "slab":
+        run_slab(args)
     else:
         run_ours(args)
 

@@ -58,7 +58,7 @@ def _clock():
 
 
 # ---- config 1: Taylor-Green vortex ---------------------------------------------------------------------------
-def config1(formats, steps=200, collision="BGK"):
+def config1(formats, steps=200, collision="BGK", graphs=True):
     """3-D Taylor-Green, 32^3, tau 0.6: E(t)/E(0) with E = 1/2 sum rho |u|^2, and the drift of the total mass per cell.
     The 3-D field is not an exact Navier-Stokes solution: exp(-2 nu |k|^2 t) is the Stokes-limit band (SURVEY.md
     section 8(c)); the FP64 run is the reference the storage formats are compared with."""
@@ -69,6 +69,7 @@ def config1(formats, steps=200, collision="BGK"):
     rows = []
     for name in ["FP64"] + [f for f in formats if f != "FP64"]:
         sim = lbm.from_workload(w, name, collision=lbm.TRT if collision == "TRT" else lbm.BGK)
+        sim.set_graphs(graphs)
         rho, u = (sim.read_rho_u_f64() if name == "FP64" else sim.read_rho_u())
         e0 = 0.5 * float((rho.astype(np.float64) * (u.astype(np.float64) ** 2).sum(0)).sum())
         m0 = float(rho.astype(np.float64).sum())
@@ -79,7 +80,7 @@ def config1(formats, steps=200, collision="BGK"):
         rows.append({"format": name, "E_over_E0": e1 / e0, "mass_drift_per_cell": (m1 - m0) / w.n_cells,
                      "steps_per_s": steps / (ms * 1e-3), "kernel": sim.kernel_name})
         sim.close()
-    return {"config": 1, "what": f"Taylor-Green 32^3, tau 0.6, {steps} steps, {collision}",
+    return {"config": 1, "what": f"Taylor-Green 32^3, tau 0.6, {steps} steps, {collision}" + ("" if graphs else ", CUDA graphs off"),
             "stokes_limit": math.exp(-2.0 * nu * k2 * steps), "rows": rows}
 
 
@@ -104,12 +105,13 @@ def l2_error(u, ref):
     return math.sqrt(float(((u - ref) ** 2).sum()) / float((ref ** 2).sum()))
 
 
-def config2(formats, steps=20000, collision="BGK"):
+def config2(formats, steps=20000, collision="BGK", graphs=True):
     lbm = _lbm()
     w = wl.poiseuille_channel()
     rows = []
     for name in formats:
         sim = lbm.from_workload(w, name, collision=lbm.TRT if collision == "TRT" else lbm.BGK)
+        sim.set_graphs(graphs)
         ms = _timed_steps(sim, steps)
         rho, u = sim.read_rho_u()
         ux = u[0].reshape(w.nz, w.ny, w.nx)[w.nz // 2, 1:-1, w.nx // 2].astype(np.float64)
@@ -118,7 +120,8 @@ def config2(formats, steps=20000, collision="BGK"):
                      "u_centre": float(ux[len(ux) // 2]), "steps_per_s": steps / (ms * 1e-3), "kernel": sim.kernel_name})
         sim.close()
     return {"config": 2, "what": f"Poiseuille 16x64x16, tau 0.8, u_max 0.01, {steps} steps, {collision}"
-                                 + (" (the slip term is BGK's; TRT with Lambda = 3/16 has none)" if collision == "TRT" else ""),
+                                 + (" (the slip term is BGK's; TRT with Lambda = 3/16 has none)" if collision == "TRT" else "")
+                                 + ("" if graphs else ", CUDA graphs off"),
             "rows": rows}
 
 
@@ -199,12 +202,13 @@ def main():
     ap.add_argument("--size", type=int, default=0)
     ap.add_argument("--collision", default="BGK", choices=["BGK", "TRT"])
     ap.add_argument("--outflow", action="store_true", help="config 4: zero-gradient outflow plane instead of equilibrium cells at x = nx-1")
+    ap.add_argument("--no-graphs", action="store_true", help="configs 1, 2: plain launches instead of CUDA graphs (lbm_set_graphs)")
     ap.add_argument("--json", default="")
     a = ap.parse_args()
     if a.config == 1:
-        res = config1((a.formats or ",".join(ALL16)).split(","), a.steps or 200, a.collision)
+        res = config1((a.formats or ",".join(ALL16)).split(","), a.steps or 200, a.collision, not a.no_graphs)
     elif a.config == 2:
-        res = config2((a.formats or ",".join(ALL16)).split(","), a.steps or 20000, a.collision)
+        res = config2((a.formats or ",".join(ALL16)).split(","), a.steps or 20000, a.collision, not a.no_graphs)
     elif a.config == 3:
         res = config3((a.formats or ",".join(ALL16)).split(","), a.size or 128, a.steps or 50000, a.collision)
     else:

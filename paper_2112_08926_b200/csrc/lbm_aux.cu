@@ -260,7 +260,8 @@ __global__ void __launch_bounds__(512) enc_table_kernel(EncEntry *tab) {
     const unsigned c0 = probe(0), c1 = (idx & 255u) == 255u ? c0 : probe(0x7FFFFFu), d = c1 - c0;
     EncEntry e;
     e.base = c0;
-    e.tmax = 0xFFFFFFFFu;
+    constexpr bool CLAMPS = PairCodec<F>::TABLE && PairCodec<F>::CHECK == 0;      // (P16_2C; see enc_by_table)
+    e.tmax = CLAMPS ? 0xFFFFFFFFu : 0u;
     unsigned add = 0;
     if (d == 0) {
         e.mult = 1u;
@@ -277,7 +278,7 @@ __global__ void __launch_bounds__(512) enc_table_kernel(EncEntry *tab) {
         const int nf = 31 - __clz((int)(sat ? d + 1 : d)), sh = 23 - nf;
         add = 1u << (sh - 1);
         e.mult = 1u << (32 - sh);
-        if (sat) e.tmax = (d << sh) | ((1u << sh) - 1u);
+        if (sat && CLAMPS) e.tmax = (d << sh) | ((1u << sh) - 1u);
     } else {
         e.mult = 0u;
 #ifdef LBM_SELFTEST_DEBUG
@@ -350,7 +351,7 @@ __global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *
                 const float r = __fmul_rn(Codec<F>::dec(c), up), r2 = __fmul_rn(Codec<F>::dec(c2), up);
                 float a, d;
                 FD::dec2(c | (c2 << 16), a, d);
-                const float e = FD::dec1((int)(short)c);
+                const float e = FD::dec1(PC::SEXT ? (int)(short)c : (int)c);
                 bad += (__float_as_uint(a) != __float_as_uint(r)) + (__float_as_uint(d) != __float_as_uint(r2)) +
                        (__float_as_uint(e) != __float_as_uint(r));
             }
@@ -358,7 +359,7 @@ __global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *
             const float r = __fmul_rn(Codec<F>::dec(c), up), r2 = __fmul_rn(Codec<F>::dec(c2), up);
             float a, d;
             PC::dec2(c | (c2 << 16), a, d);
-            const float e = PC::dec1((int)(short)c);
+            const float e = PC::dec1(PC::SEXT ? (int)(short)c : (int)c);
             const bool cn = r != r || r2 != r2;
 #ifdef LBM_SELFTEST_DEBUG
             if (!cn && __float_as_uint(a) != __float_as_uint(r)) printf("dec2lo c=%04x ref=%08x got=%08x\n", c, __float_as_uint(r), __float_as_uint(a));

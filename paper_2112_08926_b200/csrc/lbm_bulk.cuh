@@ -100,11 +100,13 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 template <int F>
 struct FullRange : PairCodec<F>::Full {
     static constexpr unsigned CHECK = PairCodec<F>::CHECK;
+    static constexpr bool SEXT = PairCodec<F>::SEXT;     // (PositFull uses the low 16 bits only: either load will do)
 };
 
 // shared-memory access (addresses are "thread base + immediate")
 __device__ __forceinline__ unsigned lds_u32(const char *p) { return *reinterpret_cast<const unsigned *>(p); }
 __device__ __forceinline__ int lds_s16(const char *p) { return (int)*reinterpret_cast<const short *>(p); }
+__device__ __forceinline__ int lds_u16(const char *p) { return (int)*reinterpret_cast<const unsigned short *>(p); }
 __device__ __forceinline__ float lds_f32(const char *p) { return *reinterpret_cast<const float *>(p); }
 
 struct TileCoord {

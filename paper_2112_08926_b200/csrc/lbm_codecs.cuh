@@ -162,7 +162,10 @@ struct Codec<F_P16_2C> {
 //             together and, if a CHECK bit shows up, decodes again with PairCodec<F>::Full (all codes, dearer).
 // Every function returns bit for bit what Codec<F>::dec / enc return (times 2^SC).
 struct EncEntry {
-    unsigned add, mult, base, tmax;     // code = base + hi32(min(bits(X) + add, tmax) * mult)
+    // code = base + hi32(min(bits(X) + add, tmax) * mult).  tmax is used by the formats that clamp (CLAMP below) and is
+    // ZERO for the others: their code is the high word of ONE 64-bit multiply-add, t * mult + {tmax = 0 : base}, whose
+    // addend is the entry's second register pair as loaded
+    unsigned add, mult, tmax, base;
 };
 
 template <int F>
@@ -170,6 +173,7 @@ struct PairCodec {
     static constexpr int SC = 0;
     static constexpr bool TABLE = false;
     static constexpr unsigned CHECK = 0;
+    static constexpr bool SEXT = false;         // dec1 wants its code sign-extended to 32 bits
     static __device__ __forceinline__ float dec1(int c) { return Codec<F>::dec((unsigned)c & 0xFFFFu); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
         a = Codec<F>::dec(w & 0xFFFFu);
@@ -186,6 +190,7 @@ struct PairHalf {
     static constexpr int SC = SCALE;
     static constexpr bool TABLE = false;
     static constexpr unsigned CHECK = 0;
+    static constexpr bool SEXT = false;
     static __device__ __forceinline__ float dec1(int c) { return __half2float(__ushort_as_half((unsigned short)c)); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
         const float2 v = __half22float2(*reinterpret_cast<const __half2 *>(&w));
@@ -213,6 +218,7 @@ struct PairCodec<F_FP16C> {
     static constexpr int SC = 0;
     static constexpr bool TABLE = false;
     static constexpr unsigned CHECK = 0;
+    static constexpr bool SEXT = true;
     static __device__ __forceinline__ float bits2f(unsigned t) {
         return __fmul_rn(__uint_as_float(t & 0x87FFF000u), __uint_as_float(0x77800000u));   // * 2^112, exact
     }
@@ -248,9 +254,10 @@ template <bool CLAMP>
 __device__ __forceinline__ unsigned enc_by_table(float X, const EncEntry *tab) {
     const unsigned xb = __float_as_uint(X);
     const uint4 e = *reinterpret_cast<const uint4 *>(tab + (xb >> 23));
-    unsigned t = xb + e.x;
-    if (CLAMP) t = min(t, e.w);
-    return __umulhi(t, e.y) + e.z;
+    const unsigned t = xb + e.x;
+    if (CLAMP) return __umulhi(min(t, e.z), e.y) + e.w;
+    const unsigned long long acc = (unsigned long long)e.z | ((unsigned long long)e.w << 32);      // e.z == 0
+    return (unsigned)(((unsigned long long)t * e.y + acc) >> 32);
 }
 
 // Decode for a regime of ZEROS (value below 1 before scaling; P16_2C has no other kind).  The 15 magnitude bits
@@ -288,6 +295,7 @@ struct PairCodec<F_P16_0S> {
     static constexpr int SC = -1;           // decoded = n 2^-22 = f / 2: one multiply, the factor 2 rides on SC
     static constexpr bool TABLE = true;
     static constexpr unsigned CHECK = 0x4000u;
+    static constexpr bool SEXT = true;
     typedef PositFull<1, 0x0B000000u, 0x02000000u, 0x0B000000u> Full;           // same scaling: f / 2
     static __device__ __forceinline__ float sm2f(unsigned t) {      // t = sign-extended code
         return __fmul_rn(__uint_as_float(t & 0x80007FFFu), __uint_as_float(0x7F000000u));   // * 2^127, exact
@@ -308,16 +316,19 @@ struct PairPositLow {
     static constexpr int SC = 0;
     static constexpr bool TABLE = true;
     static constexpr unsigned CHECK = CHK;
+    static constexpr bool SEXT = false;
     // t = the code shifted so that the magnitude sits in bits 22..8 and the sign in bit 31
     static __device__ __forceinline__ float word(unsigned t) {
         const unsigned b = __float_as_uint(__fmul_rn(__uint_as_float(t & 0x007FFF00u), __uint_as_float(0x7F000000u)));
         const unsigned v = max(b, FLOOR) * (unsigned)MUL + OFF;
         return __uint_as_float(v | (t & 0x80000000u));
     }
-    static __device__ __forceinline__ float dec1(int c) { return word((unsigned)c << 8); }     // c sign-extended
+    // one PRMT builds t from a code: bytes [0, low, high, high] -- magnitude in bits 22..8, the sign (top bit of the high
+    // byte) in bit 31; word() masks the rest
+    static __device__ __forceinline__ float dec1(int c) { return word(__byte_perm((unsigned)c, 0, 0x1104)); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
-        a = word(__byte_perm(w, 0, 0x9910) << 8);
-        b = word((unsigned)((int)w >> 8));
+        a = word(__byte_perm(w, 0, 0x1104));
+        b = word(__byte_perm(w, 0, 0x3324));
     }
     static __device__ __forceinline__ unsigned enc2(float a, float b, const EncEntry *tab) {
         return __byte_perm(enc_by_table<CHK == 0>(a, tab), enc_by_table<CHK == 0>(b, tab), 0x5410);

@@ -118,7 +118,8 @@ struct PullCell {
                 PC::dec2(w[I], a, b);
                 f[I] = J == 0 ? a : b;
             } else {
-                const int c = lds_s16(cx > 0 ? (J == 0 ? left + o : own + o) : (J == 0 ? own + o + 2 : right + o));
+                const char *at = cx > 0 ? (J == 0 ? left + o : own + o) : (J == 0 ? own + o + 2 : right + o);
+                const int c = PC::SEXT ? lds_s16(at) : lds_u16(at);      // (sign-extended only where the decoder wants it)
                 if (PC::CHECK) accs |= (unsigned)c;
                 f[I] = PC::dec1(c);
             }
