@@ -46,7 +46,7 @@ __device__ __forceinline__ void bulk_wait() {            // all but the N newest
 // ---- compile-time shape ----------------------------------------------------------------------------
 // One CTA of 16 warps per SM -- four per scheduler, 128 registers per thread, which the two-cell collision needs --
 // one loader, one storer, 14 consumers.  A tile is up to TC cells = TC/64 chunks of 32 cell pairs, one pair per lane.
-template <int Q, int F>
+template <int Q, int F, int ALT = 0>
 struct StageShape {
     typedef Elem<F> E;
     static constexpr int ES = E::SIZE;                      // bytes per stored DDF
@@ -57,14 +57,26 @@ struct StageShape {
     static constexpr int in_bytes(int tc) { return Q * (tc * ES + 2 * PAD); }
     static constexpr int out_bytes(int tc) { return Q * tc * ES; }
     static constexpr int need(int tc, int si, int so) { return si * in_bytes(tc) + so * out_bytes(tc) + TABB + HDRS * 16 + 256; }
-    static constexpr int TC = need(1024, 2, 2) <= LIMIT ? 1024 : need(512, 2, 2) <= LIMIT ? 512 : 256;   // cells per tile
+    // cells per tile: the largest of 2048 / 1024 / 768 that leaves room for THREE input stages (16-bit D2Q9: 2048, D3Q19:
+    // 1024, D3Q27: 768), else the largest that fits with two (FP32).  Measured: the third input stage
+    // is worth more than a larger tile -- unless the box's rows fill the smaller tile badly.  HAS_ALT: where the two-stage
+    // shape holds more cells (D3Q27 16-bit: 1024), it is compiled as well (ALT = 1) and stage_alt() (lbm_unit.cu) picks
+    // per box.
+    static constexpr int TC3 = need(2048, 3, 2) <= LIMIT ? 2048 : need(1024, 3, 2) <= LIMIT ? 1024 : need(768, 3, 2) <= LIMIT ? 768 : 0;
+    static constexpr int TC2 = need(1024, 2, 2) <= LIMIT ? 1024 : need(512, 2, 2) <= LIMIT ? 512 : 256;
+    static constexpr bool HAS_ALT = TC3 != 0 && TC2 > TC3;
+    static constexpr int TC = (TC3 != 0 && !(ALT == 1 && HAS_ALT)) ? TC3 : TC2;
     static constexpr int S_OUT = 2;                                                     // output stages
     static constexpr int S_IN = need(TC, 3, S_OUT) <= LIMIT ? 3 : 2;                    // input stages
     static constexpr int NCW = 14;                                                      // consumer warps
+    // D3Q27's two cells of 27 populations do not fit 128 registers together (124 bytes of spills): there a thread
+    // finishes its first cell -- pull, collide, encode, half-word stores -- before it pulls the second
+    static constexpr bool SPLIT = Q == 27;
     static constexpr int NCT = 32 * NCW, NT = NCT + 64;                                 // + the loader and the storer warp
     static constexpr int WLAG = 3;                          // the storer reports a tile written WLAG tiles later (the bulk-copy
                                                             // engine's write may take that long; waiting for it earlier stalls the storer)
-    static constexpr int LAG = WLAG + 1;                    // the list pass of a tile runs LAG tiles later
+    static constexpr int LAG = WLAG + 1;                    // the list pass of a tile runs at least LAG tiles later ...
+    static constexpr int LG = 4;                            // ... together with the lists of its group of LG consecutive tiles
     static constexpr int ROWB = TC * ES + 2 * PAD;          // one direction of one input stage
     static constexpr int INB = in_bytes(TC);
     static constexpr int OPITCH = TC * ES;                  // one direction of one output stage
@@ -78,7 +90,7 @@ struct StageShape {
     static_assert(NT == 512, "16 warps: 128 registers per thread");
     static_assert(SMEM <= LIMIT, "the CTA must fit one SM");
     static_assert(INB % 16 == 0 && ROWB % 16 == 0 && OUTB % 16 == 0 && TAB_OFF % 16 == 0 && BAR_OFF % 8 == 0, "alignment");
-    static_assert(LAG + S_IN + 2 < HDRS && LAG + 2 <= DONES, "ring sizes");
+    static_assert(LAG + LG - 1 + S_IN + 2 < HDRS && LAG + LG <= DONES, "ring sizes");
     static_assert(S_OUT >= 2, "the chunk-wise hand-over of the output stages needs two of them");
 };
 
@@ -87,9 +99,9 @@ struct StageShape {
 //   wrapped / pointing into the pads); direction I adds the immediate I * ROWB.
 // A direction without an x component is one aligned load for both cells: cell 0's pull keeps the raw word in w[I] for
 // cell 1's.
-template <int Q, int F, class PC, int J, int I>
+template <int Q, int F, int ALT, class PC, int J, int I>
 struct PullCell {
-    typedef StageShape<Q, F> SH;
+    typedef StageShape<Q, F, ALT> SH;
     // accw / accs collect the raw words / single codes for PairCodec<F>::CHECK
     static __device__ __forceinline__ void run(const char *own, const char *left, const char *right, float (&f)[Q], unsigned (&w)[Q],
                                                unsigned &accw, unsigned &accs) {
@@ -124,11 +136,11 @@ struct PullCell {
                 f[I] = PC::dec1(c);
             }
         }
-        PullCell<Q, F, PC, J, I + 1>::run(own, left, right, f, w, accw, accs);
+        PullCell<Q, F, ALT, PC, J, I + 1>::run(own, left, right, f, w, accw, accs);
     }
 };
-template <int Q, int F, class PC, int J>
-struct PullCell<Q, F, PC, J, Q> {
+template <int Q, int F, int ALT, class PC, int J>
+struct PullCell<Q, F, ALT, PC, J, Q> {
     static __device__ __forceinline__ void run(const char *, const char *, const char *, float (&)[Q], unsigned (&)[Q], unsigned &,
                                                unsigned &) {}
 };
@@ -136,19 +148,19 @@ struct PullCell<Q, F, PC, J, Q> {
 // One cell's pull with the format's cheap decoders, again with the full-range ones if a code outside their domain
 // shows up (posits: PairCodec<F>::CHECK; `wide` = the warp is in full-range mode already).  Returns whether such a
 // code was met.
-template <int Q, int F, int J>
+template <int Q, int F, int ALT, int J>
 __device__ __forceinline__ bool pull_cell(const char *own, const char *left, const char *right, float (&f)[Q], unsigned (&w)[Q], bool wide) {
     typedef PairCodec<F> PC;
     unsigned accw = 0, accs = 0;
     if constexpr (PC::CHECK != 0) {
-        if (!wide) PullCell<Q, F, PC, J, 0>::run(own, left, right, f, w, accw, accs);
+        if (!wide) PullCell<Q, F, ALT, PC, J, 0>::run(own, left, right, f, w, accw, accs);
         if (wide || (((accw >> (16 * J)) | accs) & PC::CHECK) != 0) {
             accw = accs = 0;
-            PullCell<Q, F, FullRange<F>, J, 0>::run(own, left, right, f, w, accw, accs);
+            PullCell<Q, F, ALT, FullRange<F>, J, 0>::run(own, left, right, f, w, accw, accs);
         }
         return (((accw >> (16 * J)) | accs) & PC::CHECK) != 0;
     } else {
-        PullCell<Q, F, PC, J, 0>::run(own, left, right, f, w, accw, accs);
+        PullCell<Q, F, ALT, PC, J, 0>::run(own, left, right, f, w, accw, accs);
         return false;
     }
 }
@@ -159,9 +171,9 @@ __device__ __forceinline__ bool pull_cell(const char *own, const char *left, con
 // Away from the box faces a direction's source is "tile base + per-direction constant" (BulkGeom::src_boff, in the
 // kernel's constant bank): one copy per direction for a tile of whole rows, one copy plus a 16-byte halo copy (the
 // element before / after the segment, for the directions shifted in x) for a segment of a long row.
-template <int Q, int F, int I>
+template <int Q, int F, int ALT, int I>
 struct LoadDir {
-    typedef StageShape<Q, F> SH;
+    typedef StageShape<Q, F, ALT> SH;
     static __device__ __forceinline__ void run(const char *A, const Params &p, const BulkGeom &g, const TileCoord &c, bool single,
                                                bool face, long long first_b, unsigned stage, unsigned full) {
         typedef Lat<Q> L;
@@ -197,36 +209,35 @@ struct LoadDir {
                 else bulk_g2s(dst + rowb, row + (long long)(c.x0 + c.w == p.nx ? 0 : c.x0 + c.w) * ES, SH::PAD, full);
             }
         }
-        LoadDir<Q, F, I + 1>::run(A, p, g, c, single, face, first_b, stage, full);
+        LoadDir<Q, F, ALT, I + 1>::run(A, p, g, c, single, face, first_b, stage, full);
     }
 };
-template <int Q, int F>
-struct LoadDir<Q, F, Q> {
+template <int Q, int F, int ALT>
+struct LoadDir<Q, F, ALT, Q> {
     static __device__ __forceinline__ void run(const char *, const Params &, const BulkGeom &, const TileCoord &, bool, bool, long long, unsigned,
                                                unsigned) {}
 };
 
 // hdr = the tile's slot in the header ring
-template <int Q, int F>
+template <int Q, int F, int ALT>
 __device__ __forceinline__ void stage_issue_loads(const typename Elem<F>::T *__restrict__ A, const Params &p, const BulkGeom &g,
-                                                  int t, unsigned stage, unsigned full, unsigned hdr, bool leader) {
-    typedef StageShape<Q, F> SH;
+                                                  int t, unsigned lo, unsigned hi, unsigned stage, unsigned full, unsigned hdr, bool leader) {
+    typedef StageShape<Q, F, ALT> SH;
     constexpr int ES = SH::ES;
     constexpr int n_shift = (Q == 9 ? 6 : Q == 19 ? 10 : 18);               // directions with c_x != 0
     const bool single = g.tiles_per_row == 1;
     const TileCoord c = tile_coord(t, g, p);
     const int cells = c.rows * c.w;
     if (!leader) return;
-    // the tile's header for the consumer warps: cell pairs, and the tile's slice of the flagged-cell list.  Written
-    // before the arrival below (release), read after the consumers' wait on the same barrier (acquire)
-    unsigned lo = 0, hi = 0;
-    if (p.fix_off) { lo = __ldg(p.fix_off + t); hi = __ldg(p.fix_off + t + 1); }
+    // the tile's header for the consumer warps: cell pairs, and the tile's slice [lo, hi) of the flagged-cell list (the
+    // caller read it a tile ahead: a load here would delay every tile's copies by a trip to memory).  Written before the
+    // arrival below (release), read after the consumers' wait on the same barrier (acquire)
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(hdr), "r"((unsigned)(cells >> 1)), "r"(lo), "r"(hi), "r"(0u) : "memory");
     mbar_arrive_expect_tx(full, (unsigned)(Q * cells * ES + (single ? 0 : n_shift * SH::PAD)));
     const long long first_b = ((long long)p.nx * (c.y + (long long)p.ny * c.z) + c.x0) * ES;
     // tiles on a y or z face of the box pull some directions from the opposite face (R2)
     const bool face = c.y == 0 || c.y + c.rows == p.ny || c.z == 0 || c.z == p.nz - 1;
-    LoadDir<Q, F, 0>::run(reinterpret_cast<const char *>(A), p, g, c, single, face, first_b, stage, full);
+    LoadDir<Q, F, ALT, 0>::run(reinterpret_cast<const char *>(A), p, g, c, single, face, first_b, stage, full);
 }
 
 // ---- the list pass: one flagged cell, from and to global memory ------------------------------------------------
@@ -237,26 +248,29 @@ template <int Q, int F, int I>
 struct PullMasked {
     typedef Elem<F> E;
     typedef typename E::T T;
+    // copy_from >= 0: no pull at all -- the cell takes slot I of cell `copy_from` (a fixed cell: itself; an outflow cell:
+    // its upstream neighbour), so that every kind of listed cell shares ONE batch of loads
     static __device__ __forceinline__ void run(const T *__restrict__ A, const Params &p, const long long (&rows)[3][3], int x, int xm,
-                                               int xp, unsigned mask, T (&raw)[Q]) {
+                                               int xp, unsigned mask, long long copy_from, T (&raw)[Q]) {
         typedef Lat<Q> L;
         constexpr int cx = L::c(I, 0), cy = L::c(I, 1), cz = L::c(I, 2);
         const long long own = rows[1][1] + x;
         if (I == 0) {
-            raw[0] = __ldg(A + own);
+            raw[0] = __ldg(A + (copy_from >= 0 ? copy_from : own));
         } else {
             const long long src = rows[1 - cy][1 - cz] + (cx == 0 ? x : cx > 0 ? xm : xp);
             const T *from_neighbour = A + (long long)I * p.N + src, *from_self = A + (long long)L::opp(I) * p.N + own;
-            raw[I] = __ldg(((mask >> I) & 1u) ? from_self : from_neighbour);
+            const T *from_copy = A + (long long)I * p.N + copy_from;
+            raw[I] = __ldg(copy_from >= 0 ? from_copy : ((mask >> I) & 1u) ? from_self : from_neighbour);
         }
-        PullMasked<Q, F, I + 1>::run(A, p, rows, x, xm, xp, mask, raw);
+        PullMasked<Q, F, I + 1>::run(A, p, rows, x, xm, xp, mask, copy_from, raw);
     }
 };
 template <int Q, int F>
 struct PullMasked<Q, F, Q> {
     typedef typename Elem<F>::T T;
     static __device__ __forceinline__ void run(const T *__restrict__, const Params &, const long long (&)[3][3], int, int, int, unsigned,
-                                               T (&)[Q]) {}
+                                               long long, T (&)[Q]) {}
 };
 // R9: the moving-wall term of the bounced links of a cell one of whose walls moves (bit 31 of its mask)
 template <int Q, int I>
@@ -280,22 +294,17 @@ struct MovingWallTerms<Q, Q> {
 };
 
 // fl = the cell's flag byte, mask = its `bounce` word.  A fixed cell (wall, equilibrium boundary: never updated,
-// PAPER.md:1017; R15) gets the values it has in A back; a cell next to a wall is computed again, this time with its
-// bounce-back links, with the scalar converters (bit-identical to the pair converters: lbm_codec_pair_selftest).
+// PAPER.md:1017; R15) gets the values it has in A back; an outflow cell (R18) the equilibrium of its upstream neighbour's
+// moments; a cell next to a wall is computed again, this time with its bounce-back links, with the scalar converters
+// (bit-identical to the pair converters: lbm_codec_pair_selftest).  The three kinds share their q loads and their q
+// stores -- a warp whose lanes hold cells of several kinds (a row end: wall, neighbour of the wall) waits for memory once,
+// only the arithmetic in between diverges.
 template <int Q, int F, bool FORCE, int COLL>
 __device__ __forceinline__ void fix_cell(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B, const Params &p,
                                          int x, int y, int z, unsigned fl, unsigned mask) {
     typedef Elem<F> E;
+    typedef typename E::T T;
     const long long n = x + (long long)p.nx * (y + (long long)p.ny * z);
-    if (fl & FLAG_FIXED) {
-#pragma unroll
-        for (int i = 0; i < Q; ++i) B[(long long)i * p.N + n] = __ldg(A + (long long)i * p.N + n);
-        return;
-    }
-    if (fl & FLAG_OUT) {                                                     // R18: zero-gradient outflow cell
-        outflow_cell<Q, F, FORCE>(A, B, p, n, n - x + (x == 0 ? p.nx - 1 : x - 1));
-        return;
-    }
     const int ym = y == 0 ? p.ny - 1 : y - 1, yp = y == p.ny - 1 ? 0 : y + 1;
     const int zm = z == 0 ? p.nz - 1 : z - 1, zp = z == p.nz - 1 ? 0 : z + 1;
     const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
@@ -305,42 +314,56 @@ __device__ __forceinline__ void fix_cell(const typename Elem<F>::T *__restrict__
 #pragma unroll
         for (int b = 0; b < 3; ++b) rows[a][b] = (long long)p.nx * (ys[a] + (long long)p.ny * zs[b]);
     const int xm = x == 0 ? p.nx - 1 : x - 1, xp = x == p.nx - 1 ? 0 : x + 1;
-    typename E::T raw[Q];
-    PullMasked<Q, F, 0>::run(A, p, rows, x, xm, xp, mask, raw);
-    float f[Q];
+    const long long copy_from = (fl & FLAG_FIXED) ? n : (fl & FLAG_OUT) ? n - x + xm : -1;
+    T raw[Q];
+    PullMasked<Q, F, 0>::run(A, p, rows, x, xm, xp, mask, copy_from, raw);
+    if (!(fl & FLAG_FIXED)) {
+        float f[Q];
 #pragma unroll
-    for (int i = 0; i < Q; ++i) {
-        if constexpr (E::SIZE == 4) f[i] = raw[i];
-        else f[i] = Codec<F>::dec((unsigned)raw[i]);
+        for (int i = 0; i < Q; ++i) {
+            if constexpr (E::SIZE == 4) f[i] = raw[i];
+            else f[i] = Codec<F>::dec((unsigned)raw[i]);
+        }
+        if (fl & FLAG_OUT) {                                                 // R18, as outflow_cell (lbm_kernels.cuh)
+            float rho, j[3], u[3], feq[Q];
+            moments<Q, true>(f, rho, j);
+            const float Fv[3] = {p.fx, p.fy, p.fz};
+#pragma unroll
+            for (int a = 0; a < 3; ++a) u[a] = __fdiv_rn(FORCE ? fma_(-0.5f, Fv[a], j[a]) : j[a], rho);
+            equilibrium<Q, true>(rho, u[0], u[1], u[2], feq);
+#pragma unroll
+            for (int i = 0; i < Q; ++i) f[i] = feq[i];
+        } else {
+            if (mask >> 31) MovingWallTerms<Q, 1>::run(p, rows, x, xm, xp, mask, f);
+            collide<COLL, Q, FORCE>(f, p);
+        }
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            if constexpr (E::SIZE == 4) raw[i] = f[i];
+            else raw[i] = (T)Codec<F>::enc(f[i]);
+        }
     }
-    if (mask >> 31) MovingWallTerms<Q, 1>::run(p, rows, x, xm, xp, mask, f);
-    collide<COLL, Q, FORCE>(f, p);
 #pragma unroll
-    for (int i = 0; i < Q; ++i) E::st1(B + (long long)i * p.N + n, f[i]);
+    for (int i = 0; i < Q; ++i) B[(long long)i * p.N + n] = raw[i];
 }
 
-// the flagged cells [a, b) of tile t's list, one per lane
-// (not inlined: its registers are allocated apart from the main loop's)
+// one flagged cell: entry e of the list of tile t
 template <int Q, int F, bool FORCE, int COLL>
-__device__ __forceinline__ void fix_cells_of_tile(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B,
-                                                  const Params &p, const BulkGeom &g, int t, unsigned a, unsigned b, int lane) {
+__device__ __forceinline__ void fix_list_entry(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B,
+                                               const Params &p, const BulkGeom &g, int t, uint2 e) {
     const TileCoord c = tile_coord(t, g, p);
     const FastDiv by_hw = c.last ? g.by_hw_last : g.by_hw_full;
-#pragma unroll 1
-    for (unsigned idx = a + lane; idx < b; idx += 32) {
-        const uint2 e = __ldg(p.fix_cells + idx);
-        const int ci = (int)(e.x & 0xFFFFu);                                 // cell index inside the tile
-        const int r = by_hw.div(ci >> 1), xl = ci - r * c.w;
-        fix_cell<Q, F, FORCE, COLL>(A, B, p, c.x0 + xl, c.y + r, c.z, e.x >> 16, e.y);
-    }
+    const int ci = (int)(e.x & 0xFFFFu);                                     // cell index inside the tile
+    const int r = by_hw.div(ci >> 1), xl = ci - r * c.w;
+    fix_cell<Q, F, FORCE, COLL>(A, B, p, c.x0 + xl, c.y + r, c.z, e.x >> 16, e.y);
 }
 
-template <int Q, int F, bool FORCE, int COLL = 0>
-__global__ void __launch_bounds__(StageShape<Q, F>::NT, 1)
+template <int Q, int F, bool FORCE, int COLL = 0, int ALT = 0>
+__global__ void __launch_bounds__(StageShape<Q, F, ALT>::NT, 1)
 stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename Elem<F>::T *__restrict__ B,
                              const __grid_constant__ Params p, const __grid_constant__ BulkGeom g,
                              const EncEntry *__restrict__ enc_table) {
-    typedef StageShape<Q, F> SH;
+    typedef StageShape<Q, F, ALT> SH;
     typedef Elem<F> E;
     typedef typename E::T T;
     constexpr int ES = SH::ES, S_IN = SH::S_IN, S_OUT = SH::S_OUT, NCW = SH::NCW, LAG = SH::LAG;
@@ -382,12 +405,31 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
     if (warp == NCW) {
         // ================= the loader warp =================
         const bool leader = lane == 0;
+        // the slice of the flagged-cell list of tile t, and the list entries on their way into L2 for the list pass
+        auto list_slice = [&](long long t, unsigned &lo, unsigned &hi) {
+            lo = hi = 0;
+            if (lists && leader && t < g.n_tiles) {
+                lo = __ldg(p.fix_off + t);
+                hi = __ldg(p.fix_off + t + 1);
+            }
+        };
+        auto list_prefetch = [&](unsigned lo, unsigned hi) {
+            if (leader && lo < hi) {
+                const char *a = reinterpret_cast<const char *>(p.fix_cells + lo), *b = reinterpret_cast<const char *>(p.fix_cells + hi);
+#pragma unroll 1
+                for (int n = 0; a < b && n < 8; a += 128, ++n) asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+            }
+        };
         int k = 0;
+        unsigned lo, hi;
+        list_slice(blockIdx.x, lo, hi);
 #pragma unroll 1
         for (; k < S_IN; ++k) {                                              // prologue: fill every input stage
             const long long t = (long long)blockIdx.x + (long long)k * stride;
             if (t < g.n_tiles)
-                stage_issue_loads<Q, F>(A, p, g, (int)t, smem_base + k * SH::INB, bar_full + k * 8, smem_base + SH::HDR_OFF + (k % SH::HDRS) * 16, leader);
+                stage_issue_loads<Q, F, ALT>(A, p, g, (int)t, lo, hi, smem_base + k * SH::INB, bar_full + k * 8, smem_base + SH::HDR_OFF + (k % SH::HDRS) * 16, leader);
+            list_prefetch(lo, hi);
+            list_slice(t + stride, lo, hi);
         }
         int si = 0;
         unsigned ph_in = 0;
@@ -395,7 +437,9 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
         for (long long tn = (long long)blockIdx.x + (long long)S_IN * stride; tn < g.n_tiles; tn += stride, ++k) {
             // refill the input stage of tile k - S_IN with tile k once every consumer warp has its values out of it
             mbar_wait(bar_in_empty + si * 8, ph_in);
-            stage_issue_loads<Q, F>(A, p, g, (int)tn, smem_base + si * SH::INB, bar_full + si * 8, smem_base + SH::HDR_OFF + (k % SH::HDRS) * 16, leader);
+            stage_issue_loads<Q, F, ALT>(A, p, g, (int)tn, lo, hi, smem_base + si * SH::INB, bar_full + si * 8, smem_base + SH::HDR_OFF + (k % SH::HDRS) * 16, leader);
+            list_prefetch(lo, hi);
+            list_slice(tn + stride, lo, hi);                                 // the next tile's, in flight while this warp waits
             if (++si == S_IN) { si = 0; ph_in ^= 1u; }
         }
         return;
@@ -472,11 +516,31 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                 const int right_b = own_b + 2 * ES - ((single && xl + 2 == g.tile_w) ? g.tile_w * ES : 0);   // element "xl + 2"
                 bool warp_full = false;
                 if constexpr (PC::CHECK != 0) warp_full = __any_sync(0xffffffffu, full_mode);   // one decoder per warp where possible
-                if (fp < pairs) {
+                if constexpr (SH::SPLIT) {
+                    if (fp < pairs) {
+                        float f[Q];
+                        unsigned wd[Q];
+                        char *o = ostage + 2 * fp * ES;
+                        full_mode = pull_cell<Q, F, ALT, 0>(stage + own_b, stage + left_b, stage + right_b, f, wd, warp_full);
+                        collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f, p);
+#pragma unroll
+                        for (int i = 0; i < Q; ++i) {
+                            if constexpr (ES == 4) *reinterpret_cast<float *>(o + i * SH::OPITCH) = f[i];
+                            else *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH) = (unsigned short)PC::enc1(f[i], tab);
+                        }
+                        full_mode |= pull_cell<Q, F, ALT, 1>(stage + own_b, stage + left_b, stage + right_b, f, wd, warp_full);
+                        collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f, p);
+#pragma unroll
+                        for (int i = 0; i < Q; ++i) {
+                            if constexpr (ES == 4) *reinterpret_cast<float *>(o + i * SH::OPITCH + 4) = f[i];
+                            else *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH + 2) = (unsigned short)PC::enc1(f[i], tab);
+                        }
+                    }
+                } else if (fp < pairs) {
                     float f0[Q], f1[Q];
                     unsigned wd[Q];
-                    full_mode = pull_cell<Q, F, 0>(stage + own_b, stage + left_b, stage + right_b, f0, wd, warp_full);
-                    full_mode |= pull_cell<Q, F, 1>(stage + own_b, stage + left_b, stage + right_b, f1, wd, warp_full);
+                    full_mode = pull_cell<Q, F, ALT, 0>(stage + own_b, stage + left_b, stage + right_b, f0, wd, warp_full);
+                    full_mode |= pull_cell<Q, F, ALT, 1>(stage + own_b, stage + left_b, stage + right_b, f1, wd, warp_full);
                     collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f0, p);  // the shared division (div3)
                     collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f1, p);
                     char *o = ostage + 2 * fp * ES;
@@ -493,16 +557,46 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_out_full + so * 8);
         }
-        // this chunk's share of the list pass of tile k - LAG, whose bulk store is complete by now (see the header)
+        // The list pass.  The lists of LG consecutive tiles of this CTA (a group; the last one may be shorter) are walked
+        // together, LAG tiles after the group's last tile was computed, when its bulk store is complete (`done`; stores
+        // complete in order).  A box whose every row ends in a wall has a dozen flagged cells per tile: alone they would
+        // occupy a warp -- a third of its lanes -- for a trip to memory and one collision per tile; together they fill the
+        // lanes.  The chunk ids of the tile that triggers the pass split the concatenated lists evenly, one cell per lane.
         if (lists && k >= LAG) {
-            const int j = k - LAG;
-            const uint4 hdr = *reinterpret_cast<const uint4 *>(smem + SH::HDR_OFF + (j % SH::HDRS) * 16);
-            if (hdr.y < hdr.z) {
-                const unsigned share = ((((hdr.z - hdr.y) + (1u << shift) - 1u) >> shift) + 31u) & ~31u;
-                const unsigned a = hdr.y + (unsigned)c * share, b = min(hdr.z, a + share);
-                if (a < b) {
-                    mbar_wait(bar_done + (j % SH::DONES) * 8, (unsigned)(j / SH::DONES) & 1u);
-                    fix_cells_of_tile<Q, F, FORCE, COLL>(A, B, p, g, (int)blockIdx.x + j * stride, a, b, lane);
+            const int jhi = k - LAG;
+            if (jhi % SH::LG == SH::LG - 1 || jhi == my_tiles - 1) {
+                const int jlo = jhi - jhi % SH::LG;
+                unsigned lo[SH::LG], end[SH::LG], total = 0;                 // end[g] = lists jlo .. jlo + g, concatenated
+#pragma unroll
+                for (int gi = 0; gi < SH::LG; ++gi) {
+                    lo[gi] = 0;
+                    if (jlo + gi <= jhi) {
+                        const uint4 hdr = *reinterpret_cast<const uint4 *>(smem + SH::HDR_OFF + ((jlo + gi) % SH::HDRS) * 16);
+                        lo[gi] = hdr.y;
+                        total += hdr.z - hdr.y;
+                    }
+                    end[gi] = total;
+                }
+                if (total != 0) {
+                    const unsigned share = (((total + (1u << shift) - 1u) >> shift) + 31u) & ~31u;
+                    const unsigned a = (unsigned)c * share, b = min(total, a + share);
+                    if (a < b) {
+                        mbar_wait(bar_done + (jhi % SH::DONES) * 8, (unsigned)(jhi / SH::DONES) & 1u);
+#pragma unroll 1
+                        for (unsigned v = a + lane; v < b; v += 32) {
+                            int gi = 0;
+                            unsigned first = 0;
+#pragma unroll
+                            for (int q = 0; q + 1 < SH::LG; ++q)
+                                if (v >= end[q]) { gi = q + 1; first = end[q]; }
+                            unsigned l = lo[0];
+#pragma unroll
+                            for (int q = 1; q < SH::LG; ++q)
+                                if (gi == q) l = lo[q];
+                            const uint2 e = __ldg(p.fix_cells + l + (v - first));
+                            fix_list_entry<Q, F, FORCE, COLL>(A, B, p, g, (int)blockIdx.x + (jlo + gi) * stride, e);
+                        }
+                    }
                 }
             }
         }

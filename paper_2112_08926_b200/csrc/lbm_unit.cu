@@ -64,8 +64,9 @@ cudaError_t resident_ctas(K kern, int threads, int smem, int *out, CtaCache &cac
 }
 
 // ---- the warp-specialised staged variant (lbm_stage.cuh) ----------------------------------------------
-BulkGeom stage_geom(const Params &p, long long *tiles) {
-    typedef StageShape<Q, F> SH;
+template <int ALT>
+BulkGeom stage_geom_of(const Params &p, long long *tiles) {
+    typedef StageShape<Q, F, ALT> SH;
     BulkGeom g;
     g.tile_w = p.nx <= SH::TC ? p.nx : SH::TC;
     g.tiles_per_row = (p.nx + g.tile_w - 1) / g.tile_w;
@@ -88,15 +89,27 @@ BulkGeom stage_geom(const Params &p, long long *tiles) {
     return g;
 }
 
-template <bool FORCE, int COLL = 0>
-cudaError_t launch_staged(const void *A, void *B, const Params &p, cudaStream_t st) {
-    typedef StageShape<Q, F> SH;
-    auto kern = stream_collide_staged_kernel<Q, F, FORCE, COLL>;
+// Which of the two compiled tile shapes (StageShape::HAS_ALT) a box runs with: the three-stage shape, unless the box's
+// rows fill its smaller tile so badly that the two-stage shape needs fewer than 3/4 as many tiles (D3Q27 16-bit,
+// 512-cell rows: 512 of 768 cells used against 1024 of 1024).  One rule for the kernel launch and for the per-tile lists.
+bool stage_alt(const Params &p) {
+    if (!StageShape<Q, F, 0>::HAS_ALT) return false;
+    long long t0 = 0, t1 = 0;
+    (void)stage_geom_of<0>(p, &t0);
+    (void)stage_geom_of<1>(p, &t1);
+    return 3 * t0 > 4 * t1;
+}
+BulkGeom stage_geom(const Params &p, long long *tiles) { return stage_alt(p) ? stage_geom_of<1>(p, tiles) : stage_geom_of<0>(p, tiles); }
+
+template <bool FORCE, int COLL, int ALT>
+cudaError_t launch_staged_shape(const void *A, void *B, const Params &p, cudaStream_t st) {
+    typedef StageShape<Q, F, ALT> SH;
+    auto kern = stream_collide_staged_kernel<Q, F, FORCE, COLL, ALT>;
     static CtaCache cache;
     int ctas = 0;
     if (cudaError_t e = resident_ctas(kern, SH::NT, SH::SMEM, &ctas, cache)) return e;
     long long tiles = 0;
-    const BulkGeom g = stage_geom(p, &tiles);
+    const BulkGeom g = stage_geom_of<ALT>(p, &tiles);
     if (p.nx % 16 != 0 || tiles >= 0x7FFFFFFFLL) return cudaErrorInvalidValue;
     const int grid = (int)(tiles < ctas ? tiles : ctas);
     const EncEntry *tab = nullptr;
@@ -107,6 +120,13 @@ cudaError_t launch_staged(const void *A, void *B, const Params &p, cudaStream_t 
     kern<<<grid, SH::NT, SH::SMEM, st>>>((const T *)A, (T *)B, p, g, tab);
     count_launch();
     return cudaGetLastError();
+}
+template <bool FORCE, int COLL = 0>
+cudaError_t launch_staged(const void *A, void *B, const Params &p, cudaStream_t st) {
+    if constexpr (StageShape<Q, F, 0>::HAS_ALT) {
+        if (stage_alt(p)) return launch_staged_shape<FORCE, COLL, 1>(A, B, p, st);
+    }
+    return launch_staged_shape<FORCE, COLL, 0>(A, B, p, st);
 }
 
 // Per-tile lists of flagged cell pairs for this unit's tile geometry (lbm_aux.cu)
@@ -202,7 +222,7 @@ const char *name(int V, int coll, bool force) {
 #undef LBM_KNAME
 }
 
-int staged_tile_cells() { return StageShape<Q, F>::TC; }
+int staged_tile_cells() { return StageShape<Q, F, 0>::TC; }       // (the smaller of the two shapes' tiles: the tile-count bound of pick_variant)
 
 }  // namespace
 
