@@ -153,6 +153,18 @@ int lbm_read_rho_u_f64(lbm_t *h, double *rho, double *u);
  * rho = HOST count floats, u = HOST 3*count floats (ux of all probes | uy | uz).  Synchronises. */
 int lbm_read_rho_u_at(lbm_t *h, const long long *cells, int count, float *rho, float *u);
 
+/* lbm_read_rho_u_at for callers that must not allocate device memory (code near a CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same arguments, same results, but the scratch the read-out needs on the
+ * device (the cell indices and the kernel's outputs, 24 bytes per probe) is a fixed array inside the library --
+ * LBM_STATIC_PROBES_MAX probes, 96 KiB per GPU that loads the library, held until the process exits -- instead of the
+ * handle's staging buffer.  The call makes no cudaMalloc / cudaFree and calls no allocating routine.
+ * count > LBM_STATIC_PROBES_MAX: LBM_E_INVAL, nothing is done (use lbm_read_rho_u_at, or several calls).
+ * ALL handles and threads of a process share the one array per GPU: calls that overlap on the GPU (two handles on
+ * different streams, two host threads) race on it -- serialise them.  The array keeps the last call's contents; no call
+ * depends on them.  HOST pointers; synchronises the handle's stream. */
+#define LBM_STATIC_PROBES_MAX 4096
+int lbm_read_rho_u_at_static(lbm_t *h, const long long *cells, int count, float *rho, float *u);
+
 /* Copy direction i (0 <= i < q) of the current DDF buffer, as stored (N elements of 2, 4 or 8 bytes),
  * to a HOST pointer.  Synchronises.  For bit-level parity tests. */
 int lbm_read_ddf(lbm_t *h, int i, void *out);

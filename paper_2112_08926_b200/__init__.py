@@ -30,6 +30,7 @@ FORMATS = {"FP32": 0, "FP16S": 1, "FP16C": 2, "P16_0S": 3, "P16_1S": 4, "P16_2C"
 FORMAT_NAMES = {v: k for k, v in FORMATS.items()}
 FLAG_WALL, FLAG_EQ, FLAG_OUT = 0x01, 0x02, 0x04
 VARIANT_AUTO, VARIANT_BULK, VARIANT_STAGED = 0, 16, 32
+STATIC_PROBES_MAX = 4096           # include/lbm.h LBM_STATIC_PROBES_MAX
 OK, E_INVAL, E_UNSUPPORTED, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/lbm.h declares: (restype, argtypes)
@@ -51,6 +52,7 @@ SYMBOLS = {
     "lbm_read_rho_u_device": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_f64": (_i, [_p, _p, _p]),
     "lbm_read_rho_u_at": (_i, [_p, _p, _i, _p, _p]),
+    "lbm_read_rho_u_at_static": (_i, [_p, _p, _i, _p, _p]),
     "lbm_read_ddf": (_i, [_p, _i, _p]),
     "lbm_sync": (_i, [_p]),
     "lbm_steps_done": (_ll, [_p]),
@@ -261,6 +263,15 @@ class Simulation:
         rho = np.empty(cells.size, np.float32)
         u = np.empty((3, cells.size), np.float32)
         _check(lib().lbm_read_rho_u_at(self._h, _np_ptr(cells), cells.size, _np_ptr(rho), _np_ptr(u)))
+        return rho, u
+
+    def read_rho_u_at_static(self, cells):
+        """read_rho_u_at without any device allocation: the scratch is a fixed array in the library (at most
+        STATIC_PROBES_MAX cells per call; shared by all handles -- do not overlap calls).  include/lbm.h."""
+        cells = np.ascontiguousarray(cells, dtype=np.int64).reshape(-1)
+        rho = np.empty(cells.size, np.float32)
+        u = np.empty((3, cells.size), np.float32)
+        _check(lib().lbm_read_rho_u_at_static(self._h, _np_ptr(cells), cells.size, _np_ptr(rho), _np_ptr(u)))
         return rho, u
 
     def read_ddf(self, i: int) -> np.ndarray:

@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -486,6 +487,61 @@ int lbm_read_rho_u_at(lbm_t *h, const long long *cells, int count, float *rho, f
     const size_t cb = (size_t)count * 8, fb = (size_t)count * 16;
     if (int rc = ensure_scratch(h, cb + fb)) return rc;
     char *d = (char *)h->scratch;
+    float *df = (float *)(d + cb);
+    cudaError_t e = cudaMemcpyAsync(d, cells, cb, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = h->ops->probe(h->ddf[h->cur], make_params(h), h->has_force, (const long long *)d, count, df, df + count, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rho, df, (size_t)count * 4, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(u, df + count, (size_t)count * 12, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e2 = cudaStreamSynchronize(h->stream);
+    LBM_CUDA_TRY(e);
+    LBM_CUDA_TRY(e2);
+    return LBM_OK;
+}
+
+}  // extern "C"
+
+// ---- lbm_read_rho_u_at_static: the probe read-out for callers that must not allocate ---------------------------
+// The scratch of lbm_read_rho_u_at (the cell indices on the device + the kernel's outputs) comes from the handle's
+// staging buffer, i.e. from cudaMalloc at the first call and whenever a call needs more.  Here it is a fixed array in the
+// library's image: 24 bytes per probe (8-byte cell index | rho | ux | uy | uz), LBM_STATIC_PROBES_MAX probes, 96 KiB
+// that every GPU which loads the library holds until the process exits.
+// In host code the array's NAME is a host-side stand-in, not a device address: its address comes from
+// cudaGetSymbolAddress, asked once per device with that device current (the array exists once per device).
+static __device__ __align__(256) unsigned char g_static_probe_scratch[LBM_STATIC_PROBES_MAX * 24];
+
+namespace {
+int static_probe_scratch(int device, unsigned char **out) {          // the caller has made `device` current (enter())
+    static std::mutex mu;
+    static unsigned char *addr[64];
+    if (device < 0 || device >= 64) return fail(LBM_E_INVAL, "lbm_read_rho_u_at_static: device ordinal out of range");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[device]) {
+        void *ptr = nullptr;
+        LBM_CUDA_TRY(cudaGetSymbolAddress(&ptr, g_static_probe_scratch));
+        addr[device] = (unsigned char *)ptr;
+    }
+    *out = addr[device];
+    return LBM_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int lbm_read_rho_u_at_static(lbm_t *h, const long long *cells, int count, float *rho, float *u) {
+    if (int rc = enter(h)) return rc;
+    if (!h->inited) return fail(LBM_E_STATE, "lbm_read_rho_u_at_static: call lbm_init first");
+    if (count < 0 || (count > 0 && (!cells || !rho || !u))) return fail(LBM_E_INVAL, "lbm_read_rho_u_at_static: bad arguments");
+    if (count > LBM_STATIC_PROBES_MAX)
+        return fail(LBM_E_INVAL, "lbm_read_rho_u_at_static: count = " + std::to_string(count) + " exceeds LBM_STATIC_PROBES_MAX = " +
+                                     std::to_string(LBM_STATIC_PROBES_MAX) + " (the fixed scratch array; use lbm_read_rho_u_at)");
+    if (count == 0) return LBM_OK;
+    for (int k = 0; k < count; ++k)
+        if (cells[k] < 0 || cells[k] >= h->N) return fail(LBM_E_INVAL, "lbm_read_rho_u_at_static: cell index out of range");
+    unsigned char *d = nullptr;
+    if (int rc = static_probe_scratch(h->device, &d)) return rc;
+    // layout: count cell indices, then rho [count], then u [3][count].  The array keeps the last call's contents; nothing
+    // here must start at zero: the copy below and the kernel overwrite every byte that is read afterwards.
+    const size_t cb = (size_t)count * 8;
     float *df = (float *)(d + cb);
     cudaError_t e = cudaMemcpyAsync(d, cells, cb, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) e = h->ops->probe(h->ddf[h->cur], make_params(h), h->has_force, (const long long *)d, count, df, df + count, h->stream);
