@@ -42,6 +42,11 @@ template <int N>
 __device__ __forceinline__ void bulk_wait() {            // all but the N newest groups are complete (written)
     asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
 }
+// Orders this thread's accesses through the async proxy (the bulk-copy engine) and through the generic proxy (ordinary
+// loads / stores) to the same GLOBAL addresses.  The list pass overwrites, with ordinary stores, cells that a bulk store
+// wrote: without the fence on the way from "the bulk store is complete" to "the ordinary store is issued" the bulk
+// store's data can still land last (seen on FP32 boxes, whose stores drain slowest: about one tile in 2*10^7).
+__device__ __forceinline__ void fence_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
 // ---- compile-time shape ----------------------------------------------------------------------------
 // One CTA of 16 warps per SM -- four per scheduler, 128 registers per thread, which the two-cell collision needs --
@@ -465,6 +470,7 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                 mbar_arrive(bar_out_empty + so * 8);
                 if (lists && k >= SH::WLAG) {
                     bulk_wait<SH::WLAG>();                                   // tile k - WLAG is written
+                    fence_async_global();
                     mbar_arrive(bar_done + ((k - SH::WLAG) % SH::DONES) * 8);
                 }
             }
@@ -473,6 +479,7 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
         }
         if (leader) {
             bulk_wait<0>();                                                  // all stores complete before the CTA's shared memory goes
+            fence_async_global();
             if (lists)
                 for (int j = k > SH::WLAG ? k - SH::WLAG : 0; j < k; ++j) mbar_arrive(bar_done + (j % SH::DONES) * 8);
         }
@@ -566,6 +573,13 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
             const int jhi = k - LAG;
             if (jhi % SH::LG == SH::LG - 1 || jhi == my_tiles - 1) {
                 const int jlo = jhi - jhi % SH::LG;
+                // The headers of the group must be there before they are read.  A chunk of a real tile k has waited for
+                // `full` of tile k, which the loader signals after it wrote header k, hence after the headers of all earlier
+                // tiles.  A chunk id of one of the LAG trailing pseudo-tiles has waited for nothing: a warp that runs ahead
+                // of a lagging loader (FP32 boxes: the kernel waits for memory) would read the ring slot's previous
+                // content -- some other tile's list bounds.  `done` of tile jhi implies the header (header -> full ->
+                // computed -> stored -> done), so these chunks wait for it first.
+                if (k >= my_tiles) mbar_wait(bar_done + (jhi % SH::DONES) * 8, (unsigned)(jhi / SH::DONES) & 1u);
                 unsigned lo[SH::LG], end[SH::LG], total = 0;                 // end[g] = lists jlo .. jlo + g, concatenated
 #pragma unroll
                 for (int gi = 0; gi < SH::LG; ++gi) {
@@ -582,6 +596,7 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                     const unsigned a = (unsigned)c * share, b = min(total, a + share);
                     if (a < b) {
                         mbar_wait(bar_done + (jhi % SH::DONES) * 8, (unsigned)(jhi / SH::DONES) & 1u);
+                        fence_async_global();
 #pragma unroll 1
                         for (unsigned v = a + lane; v < b; v += 32) {
                             int gi = 0;

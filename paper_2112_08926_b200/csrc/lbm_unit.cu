@@ -68,8 +68,10 @@ template <int ALT>
 BulkGeom stage_geom_of(const Params &p, long long *tiles) {
     typedef StageShape<Q, F, ALT> SH;
     BulkGeom g;
-    g.tile_w = p.nx <= SH::TC ? p.nx : SH::TC;
-    g.tiles_per_row = (p.nx + g.tile_w - 1) / g.tile_w;
+    // a row longer than a tile is cut into EQUAL pieces (multiples of 16 cells; the last one may be shorter): 1280 cells
+    // are 2 x 640, not 1024 + 256 -- a short tile costs the same per-tile work and leaves the stages half empty
+    g.tiles_per_row = (p.nx + SH::TC - 1) / SH::TC;
+    g.tile_w = p.nx <= SH::TC ? p.nx : ((p.nx + g.tiles_per_row - 1) / g.tiles_per_row + 15) / 16 * 16;
     g.rows_per_tile = g.tiles_per_row == 1 ? SH::TC / p.nx : 1;
     const int w_last = p.nx - (g.tiles_per_row - 1) * g.tile_w;
     g.by_hw_full = FastDiv::make(g.tile_w / 2);
