@@ -81,7 +81,10 @@ struct StageShape {
     static constexpr int WLAG = 3;                          // the storer reports a tile written WLAG tiles later (the bulk-copy
                                                             // engine's write may take that long; waiting for it earlier stalls the storer)
     static constexpr int LAG = WLAG + 1;                    // the list pass of a tile runs at least LAG tiles later ...
-    static constexpr int LG = 4;                            // ... together with the lists of its group of LG consecutive tiles
+    // ... together with the lists of its group of LG consecutive tiles.  Measured (cavity 256^3): grouping gives the
+    // instruction-bound 16-bit kernels +2% (FP16S) to +34% (P16_1S) and costs the FP32 kernel, which waits for memory
+    // anyway, 8% -- FP32 keeps one list per pass
+    static constexpr int LG = ES == 4 ? 1 : 4;
     static constexpr int ROWB = TC * ES + 2 * PAD;          // one direction of one input stage
     static constexpr int INB = in_bytes(TC);
     static constexpr int OPITCH = TC * ES;                  // one direction of one output stage
