@@ -73,10 +73,15 @@ struct StageShape {
     static constexpr int TC = (TC3 != 0 && !(ALT == 1 && HAS_ALT)) ? TC3 : TC2;
     static constexpr int S_OUT = 2;                                                     // output stages
     static constexpr int S_IN = need(TC, 3, S_OUT) <= LIMIT ? 3 : 2;                    // input stages
-    static constexpr int NCW = 14;                                                      // consumer warps
-    // D3Q27's two cells of 27 populations do not fit 128 registers together (124 bytes of spills): there a thread
-    // finishes its first cell -- pull, collide, encode, half-word stores -- before it pulls the second
-    static constexpr bool SPLIT = Q == 27;
+    // consumer warps: 14 (+ loader + storer = 16 warps, 128 registers per thread).  The D3Q19 posits run 18 + 2 warps of 96
+    // registers instead: their encoder-table reads keep the shared-memory pipe 79% busy and the warps waiting on it
+    // (profiles/r02b_staged_kernels.md), and four more warps hide more of that than the 40 spilled bytes cost (+4-8%)
+    static constexpr bool MANY = PairCodec<F>::TABLE && Q == 19;
+    static constexpr int NCW = MANY ? 18 : 14;
+    // D3Q27's two cells of 27 populations do not fit 128 registers together (124 bytes of spills): there -- and in the
+    // 96-register posit kernels -- a thread finishes its first cell (pull, collide, encode, half-word stores) before it
+    // pulls the second
+    static constexpr bool SPLIT = Q == 27 || MANY;
     static constexpr int NCT = 32 * NCW, NT = NCT + 64;                                 // + the loader and the storer warp
     static constexpr int WLAG = 3;                          // the storer reports a tile written WLAG tiles later (the bulk-copy
                                                             // engine's write may take that long; waiting for it earlier stalls the storer)
@@ -95,7 +100,7 @@ struct StageShape {
     static constexpr int BAR_OFF = HDR_OFF + HDRS * 16;     // full[S_IN], in_empty[S_IN], out_full[S_OUT], out_empty[S_OUT], done[DONES]
     static constexpr int CTR_OFF = BAR_OFF + (2 * (S_IN + S_OUT) + DONES) * 8;          // the chunk counter
     static constexpr int SMEM = CTR_OFF + 8;
-    static_assert(NT == 512, "16 warps: 128 registers per thread");
+    static_assert(NT == (MANY ? 640 : 512), "16 warps: 128 registers per thread (20: 96)");
     static_assert(SMEM <= LIMIT, "the CTA must fit one SM");
     static_assert(INB % 16 == 0 && ROWB % 16 == 0 && OUTB % 16 == 0 && TAB_OFF % 16 == 0 && BAR_OFF % 8 == 0, "alignment");
     static_assert(LAG + LG - 1 + S_IN + 2 < HDRS && LAG + LG <= DONES, "ring sizes");
