@@ -151,7 +151,11 @@ def test_mass_conservation_fp32():
 # copies, wrap at the row ends), the smallest legal row (16 cells), 2-D
 BULK_SHAPES = [(19, (64, 5, 3)), (19, (560, 3, 2)), (19, (1040, 2, 2)), (19, (16, 4, 5)), (19, (512, 2, 1)), (19, (1024, 3, 2)),
                (19, (2064, 2, 1)),
-               (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1))]
+               (27, (272, 3, 3)), (27, (32, 4, 4)), (9, (48, 9, 1)), (9, (1056, 3, 1)),
+               # round 2: the 768-cell (three input stages) and 1024-cell (two) tile shapes of 16-bit D3Q27 -- exactly one
+               # tile per row, two rows per 1024-cell tile with a ragged last tile, three rows per 768-cell tile --, the
+               # 2048-cell tiles of 16-bit D2Q9 (one row, many rows, a long row in three equal pieces)
+               (27, (768, 3, 2)), (27, (512, 5, 3)), (27, (256, 7, 3)), (9, (2048, 5, 1)), (9, (64, 70, 1)), (9, (4112, 3, 1))]
 
 
 STAGED = [(lbm.VARIANT_STAGED, "staged")]
@@ -168,7 +172,7 @@ def test_bulk_variant_periodic(q, shape, name, variant, tag):
 
 
 @pytest.mark.parametrize("q,shape", [(19, (48, 7, 5)), (19, (544, 3, 3)), (19, (1040, 3, 2)), (27, (32, 6, 5)), (27, (1072, 2, 2)),
-                                     (9, (64, 11, 1))])
+                                     (9, (64, 11, 1)), (27, (512, 5, 3)), (27, (256, 7, 3)), (9, (2048, 5, 1)), (9, (64, 70, 1))])
 @pytest.mark.parametrize("name", ALL_FORMATS)
 @pytest.mark.parametrize("variant,tag", STAGED)
 def test_bulk_variant_walls_moving_walls_force(q, shape, name, variant, tag):
