@@ -73,7 +73,7 @@ bool valid_velset(int v) { return v == LBM_D2Q9 || v == LBM_D3Q19 || v == LBM_D3
 bool valid_format(int f) { return f >= LBM_FP32 && f <= LBM_FP64_FP32; }
 
 Params make_params(const lbm *h) {
-    Params p;
+    Params p = {};
     p.nx = h->nx; p.ny = h->ny; p.nz = h->nz;
     p.N = h->N;
     p.omega = h->omega;

@@ -92,14 +92,15 @@ BulkGeom stage_geom_of(const Params &p, long long *tiles) {
 }
 
 // Which of the two compiled tile shapes (StageShape::HAS_ALT) a box runs with: the three-stage shape, unless the box's
-// rows fill its smaller tile so badly that the two-stage shape needs fewer than 3/4 as many tiles (D3Q27 16-bit,
-// 512-cell rows: 512 of 768 cells used against 1024 of 1024).  One rule for the kernel launch and for the per-tile lists.
+// rows fill its smaller tile so badly that the two-stage shape's tiles hold at least 1.5 times the cells.  Measured, D3Q27
+// FP16S cubes, fraction of the HBM roofline with the 768 x 3 | 1024 x 2 shape: 256^3 (768 | 1024 cells per tile) 0.85 |
+// 0.75, 320^3 (640 | 960) 0.77 | 0.77, 384^3 (768 | 768) 0.86 | 0.73, 448^3 (448 | 896) 0.62 | 0.79, 512^3 (512 | 1024)
+// 0.70 | 0.79.  One rule for the kernel launch and for the per-tile lists.
 bool stage_alt(const Params &p) {
     if (!StageShape<Q, F, 0>::HAS_ALT) return false;
     long long t0 = 0, t1 = 0;
-    (void)stage_geom_of<0>(p, &t0);
-    (void)stage_geom_of<1>(p, &t1);
-    return 3 * t0 > 4 * t1;
+    const BulkGeom g0 = stage_geom_of<0>(p, &t0), g1 = stage_geom_of<1>(p, &t1);
+    return 2LL * g1.rows_per_tile * g1.tile_w >= 3LL * g0.rows_per_tile * g0.tile_w;
 }
 BulkGeom stage_geom(const Params &p, long long *tiles) { return stage_alt(p) ? stage_geom_of<1>(p, tiles) : stage_geom_of<0>(p, tiles); }
 
@@ -139,7 +140,9 @@ cudaError_t build_fix_lists(const Params &p, unsigned **off_out, uint2 **list_ou
     return build_fix_lists_for(p, g, off_out, list_out, st);
 }
 
-cudaError_t stream_collide(const void *A, void *B, const Params &p, int V, int coll, bool force, cudaStream_t st) {
+cudaError_t stream_collide(const void *A, void *B, const Params &p_in, int V, int coll, bool force, cudaStream_t st) {
+    Params p = p_in;
+    if (force) guo_constants<Q>(p);                          // R10's per-direction constants (lbm_lattice.cuh)
     if (!p.shifted) {
         // R17, the paper's negative control (eqs (19)-(23)): the per-thread kernel, one cell per thread
         if (coll == 1) return force ? launch_sc<1, true, 1, false>(A, B, p, st) : launch_sc<1, false, 1, false>(A, B, p, st);
