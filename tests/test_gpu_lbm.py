@@ -516,3 +516,33 @@ def test_staged_kernel_equals_per_thread_kernel_over_a_long_run(name, steps):
         assert torch.equal(ta, tb), (name, "first difference by step", done)
     a.close()
     b.close()
+
+
+def _long_run_boxes():
+    w1 = wl.karman_vortex_street(512, 128, 32, radius=8.0)
+    w2 = wl.poiseuille_channel(128, 128, 64)
+    w3 = wl.random_walls(wl.perturbed_equilibrium(256, 96, 64, seed=5, tau=0.7), 0.05, seed=7, moving_fraction=0.5)
+    w3.force = (1e-5, -2e-5, 3e-5)
+    w4 = wl.lid_driven_cavity(96, velset=27)
+    w5 = wl.random_walls(wl.perturbed_equilibrium(2048, 512, 1, seed=9, velset=9, tau=0.7), 0.02, seed=11, moving_fraction=0.5)
+    w6 = wl.random_walls(wl.perturbed_equilibrium(1280, 64, 16, seed=13, tau=0.7), 0.02, seed=15)
+    return {"karman": w1, "poiseuille_force": w2, "random_walls_force": w3, "cavity_d3q27": w4, "d2q9_walls": w5, "long_rows": w6}
+
+
+# The same long-run comparison on the other kinds of box (equilibrium rim, body force, random and moving walls, D3Q27,
+# D2Q9 with 2048-cell tiles, rows cut into several tiles), FP32 -- the storage whose kernel waits for memory and therefore
+# shows a wrong hand-over first -- and one 16-bit format.
+@pytest.mark.parametrize("box", ["karman", "poiseuille_force", "random_walls_force", "cavity_d3q27", "d2q9_walls", "long_rows"])
+@pytest.mark.parametrize("name", ["FP32", "FP16C"])
+def test_staged_kernel_equals_per_thread_kernel_long_run_other_boxes(box, name):
+    import torch
+    w = _long_run_boxes()[box]
+    a = lbm.from_workload(w, name, variant=lbm.VARIANT_STAGED)
+    b = lbm.from_workload(w, name, variant=2)
+    assert "staged" in a.kernel_name and "staged" not in b.kernel_name
+    for done in range(512, 4096 + 1, 512):
+        a.step(512)
+        b.step(512)
+        assert torch.equal(a._keep[a.steps_done & 1], b._keep[b.steps_done & 1]), (box, name, "first difference by step", done)
+    a.close()
+    b.close()
