@@ -58,7 +58,10 @@ struct StageShape {
     static constexpr int PAD = 16;                          // halo pad in front of and behind every input segment
     static constexpr int LIMIT = 227 * 1024 - 1024;         // one CTA per SM
     static constexpr int TABB = PairCodec<F>::TABLE ? 512 * 16 : 0;
-    static constexpr int HDRS = 16, DONES = 8;              // rings: tile headers (16 bytes each), "tile stored" barriers
+    // rings: tile headers (16 bytes each), "tile stored" barriers.  A `done` barrier is waited on by phase parity, so a
+    // waiter must test it before its slot has completed a second time, i.e. before the storer is DONES + WLAG - LAG tiles
+    // past the waiter's tile: 15 tiles with 16 slots, far beyond what the stage hand-over lets the warps drift apart
+    static constexpr int HDRS = 16, DONES = 16;
     static constexpr int in_bytes(int tc) { return Q * (tc * ES + 2 * PAD); }
     static constexpr int out_bytes(int tc) { return Q * tc * ES; }
     static constexpr int need(int tc, int si, int so) { return si * in_bytes(tc) + so * out_bytes(tc) + TABB + HDRS * 16 + 256; }
@@ -103,6 +106,7 @@ struct StageShape {
     static_assert(NT == (MANY ? 640 : 512), "16 warps: 128 registers per thread (20: 96)");
     static_assert(SMEM <= LIMIT, "the CTA must fit one SM");
     static_assert(INB % 16 == 0 && ROWB % 16 == 0 && OUTB % 16 == 0 && TAB_OFF % 16 == 0 && BAR_OFF % 8 == 0, "alignment");
+    static_assert((2 * (S_IN + S_OUT) + DONES) * 8 + 8 <= 256, "the barriers fit the 256 bytes need() reserves for them");
     static_assert(LAG + LG - 1 + S_IN + 2 < HDRS && LAG + LG <= DONES, "ring sizes");
     static_assert(S_OUT >= 2, "the chunk-wise hand-over of the output stages needs two of them");
 };
