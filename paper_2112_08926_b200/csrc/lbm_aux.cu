@@ -341,6 +341,15 @@ __global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *
         const unsigned w2 = PC::enc2(__fmul_rn(other, up), __fmul_rn(x, up), tab);
         const bool nan = x != x || other != other;                              // NaN payloads of binary16 are not pinned
         if (!nan) bad += (w1 != (ref | (ref_o << 16))) + (w2 != (ref_o | (ref << 16)));
+        if constexpr (PC::FAST) {                                               // the table-free encoder, wherever it claims to be valid
+            unsigned acc = 0;
+            const unsigned w3 = PC::enc2_fast(__fmul_rn(x, up), __fmul_rn(other, up), acc);
+            if (!nan && !(acc & PC::FAST_BAD)) bad += w3 != (ref | (ref_o << 16));
+            acc = 0;
+            const unsigned w4 = PC::enc2_fast(__fmul_rn(x, up), __fmul_rn(x, up), acc);
+            // (and it must claim validity on the whole regime of zeros: |2^7 x| < 1)
+            if (!nan && (b & 0x7FFFFFFFu) < 0x3BFFF000u /* just below 2^-7 */) bad += (acc & PC::FAST_BAD) != 0 || w4 != (ref | (ref << 16));
+        }
 #ifdef LBM_SELFTEST_DEBUG
         if (!nan && (w1 & 0xFFFFu) != ref && (b % 977u) == 0) printf("enc x=%08x ref=%04x got=%04x\n", b, ref, w1 & 0xFFFFu);
 #endif

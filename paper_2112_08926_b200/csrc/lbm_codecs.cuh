@@ -174,6 +174,7 @@ struct PairCodec {
     static constexpr bool TABLE = false;
     static constexpr unsigned CHECK = 0;
     static constexpr bool SEXT = false;         // dec1 wants its code sign-extended to 32 bits
+    static constexpr bool FAST = false;         // enc2_fast exists (a table-free encoder for part of the range)
     static __device__ __forceinline__ float dec1(int c) { return Codec<F>::dec((unsigned)c & 0xFFFFu); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
         a = Codec<F>::dec(w & 0xFFFFu);
@@ -191,6 +192,7 @@ struct PairHalf {
     static constexpr bool TABLE = false;
     static constexpr unsigned CHECK = 0;
     static constexpr bool SEXT = false;
+    static constexpr bool FAST = false;         // enc2_fast exists (a table-free encoder for part of the range)
     static __device__ __forceinline__ float dec1(int c) { return __half2float(__ushort_as_half((unsigned short)c)); }
     static __device__ __forceinline__ void dec2(unsigned w, float &a, float &b) {
         const float2 v = __half22float2(*reinterpret_cast<const __half2 *>(&w));
@@ -219,6 +221,7 @@ struct PairCodec<F_FP16C> {
     static constexpr bool TABLE = false;
     static constexpr unsigned CHECK = 0;
     static constexpr bool SEXT = true;
+    static constexpr bool FAST = false;         // enc2_fast exists (a table-free encoder for part of the range)
     static __device__ __forceinline__ float bits2f(unsigned t) {
         return __fmul_rn(__uint_as_float(t & 0x87FFF000u), __uint_as_float(0x77800000u));   // * 2^112, exact
     }
@@ -296,6 +299,7 @@ struct PairCodec<F_P16_0S> {
     static constexpr bool TABLE = true;
     static constexpr unsigned CHECK = 0x4000u;
     static constexpr bool SEXT = true;
+    static constexpr bool FAST = true;
     typedef PositFull<1, 0x0B000000u, 0x02000000u, 0x0B000000u> Full;           // same scaling: f / 2
     static __device__ __forceinline__ float sm2f(unsigned t) {      // t = sign-extended code
         return __fmul_rn(__uint_as_float(t & 0x80007FFFu), __uint_as_float(0x7F000000u));   // * 2^127, exact
@@ -309,6 +313,24 @@ struct PairCodec<F_P16_0S> {
         return __byte_perm(enc_by_table<false>(a, tab), enc_by_table<false>(b, tab), 0x5410);
     }
     static __device__ __forceinline__ unsigned enc1(float a, const EncEntry *tab) { return enc_by_table<false>(a, tab) & 0xFFFFu; }
+    // The table-free encoder for a regime of zeros.  Below 1 a posit with es = 0 is FIXED POINT -- the magnitude code n is
+    // the value 2^7 |f| in units of 2^-14 (the decoder above uses the same fact) -- so rule U (nearest value, ties to the
+    // larger magnitude, R14) is n = floor(2^21 |f| + 1/2) = floor(2^22 |X| + 1/2) for X = f / 2 (SC = -1).  Two FP32
+    // operations rounded TOWARDS ZERO compute it exactly: s = fma.rz(|X|, 2^22, 1/2) is the largest float <= the true sum,
+    // so it never crosses an integer downwards (integers below 2^24 are floats); fadd.rz(s, 2^23) leaves floor(s) in the
+    // mantissa.  (Round-to-nearest would fail: 2^22 |X| = 1/2 - 2^-25 gives 1 - 2^-25, a tie that rounds up to 1.)
+    // No shared-memory table read, no integer pipe.  `acc` collects every bit above bit 13 of the results: if any is set
+    // -- |2^7 f| >= 1, a regime of ones, or a NaN -- the caller encodes again with enc2 (the table).  Checked against
+    // Codec<F_P16_0S>::enc on all 2^32 inputs by lbm_codec_pair_selftest.
+    static __device__ __forceinline__ unsigned enc2_fast(float a, float b, unsigned &acc) {
+        const float sa = __fmaf_rz(fabsf(a), 4194304.0f, 0.5f), sb = __fmaf_rz(fabsf(b), 4194304.0f, 0.5f);
+        const unsigned ta = __float_as_uint(__fadd_rz(sa, 8388608.0f)) ^ 0x4B000000u;       // = n while n < 2^23
+        const unsigned tb = __float_as_uint(__fadd_rz(sb, 8388608.0f)) ^ 0x4B000000u;
+        acc |= ta | tb;
+        const unsigned signs = __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x7632);
+        return __byte_perm(ta, tb, 0x5410) | (signs & 0x80008000u);
+    }
+    static constexpr unsigned FAST_BAD = 0xFFFFC000u;       // acc & FAST_BAD != 0: outside enc2_fast's domain
 };
 
 template <int MUL, unsigned OFF, unsigned FLOOR, unsigned CHK>
@@ -317,6 +339,7 @@ struct PairPositLow {
     static constexpr bool TABLE = true;
     static constexpr unsigned CHECK = CHK;
     static constexpr bool SEXT = false;
+    static constexpr bool FAST = false;         // enc2_fast exists (a table-free encoder for part of the range)
     // t = the code shifted so that the magnitude sits in bits 22..8 and the sign in bit 31
     static __device__ __forceinline__ float word(unsigned t) {
         const unsigned b = __float_as_uint(__fmul_rn(__uint_as_float(t & 0x007FFF00u), __uint_as_float(0x7F000000u)));

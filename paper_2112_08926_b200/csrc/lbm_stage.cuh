@@ -79,7 +79,7 @@ struct StageShape {
     // consumer warps: 14 (+ loader + storer = 16 warps, 128 registers per thread).  The D3Q19 posits run 18 + 2 warps of 96
     // registers instead: their encoder-table reads keep the shared-memory pipe 79% busy and the warps waiting on it
     // (profiles/r02b_staged_kernels.md), and four more warps hide more of that than the 40 spilled bytes cost (+4-8%)
-    static constexpr bool MANY = PairCodec<F>::TABLE && Q == 19;
+    static constexpr bool MANY = PairCodec<F>::TABLE && !PairCodec<F>::FAST && Q == 19;
     static constexpr int NCW = MANY ? 18 : 14;
     // D3Q27's two cells of 27 populations do not fit 128 registers together (124 bytes of spills): there -- and in the
     // 96-register posit kernels -- a thread finishes its first cell (pull, collide, encode, half-word stores) before it
@@ -563,10 +563,26 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                     collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f0, p);  // the shared division (div3)
                     collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f1, p);
                     char *o = ostage + 2 * fp * ES;
+                    if constexpr (PC::FAST) {
+                        // the table-free encoder (P16_0S below 2^-7: every DDF of a flow at LBM velocities); should a value
+                        // fall outside its domain, the pair's words are encoded again with the table
+                        // (a thread whose inputs needed the full-range decoder goes to the table directly: its results are
+                        // of the same size)
+                        unsigned acc = full_mode ? PC::FAST_BAD : 0u;
+                        if (!full_mode) {
 #pragma unroll
-                    for (int i = 0; i < Q; ++i) {
-                        if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + i * SH::OPITCH) = make_float2(f0[i], f1[i]);
-                        else *reinterpret_cast<unsigned *>(o + i * SH::OPITCH) = PC::enc2(f0[i], f1[i], tab);
+                            for (int i = 0; i < Q; ++i) *reinterpret_cast<unsigned *>(o + i * SH::OPITCH) = PC::enc2_fast(f0[i], f1[i], acc);
+                        }
+                        if (acc & PC::FAST_BAD) {
+#pragma unroll
+                            for (int i = 0; i < Q; ++i) *reinterpret_cast<unsigned *>(o + i * SH::OPITCH) = PC::enc2(f0[i], f1[i], tab);
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < Q; ++i) {
+                            if constexpr (ES == 4) *reinterpret_cast<float2 *>(o + i * SH::OPITCH) = make_float2(f0[i], f1[i]);
+                            else *reinterpret_cast<unsigned *>(o + i * SH::OPITCH) = PC::enc2(f0[i], f1[i], tab);
+                        }
                     }
                 }
             }
