@@ -346,6 +346,9 @@ __global__ void __launch_bounds__(256) pair_selftest_kernel(unsigned long long *
             const unsigned w3 = PC::enc2_fast(__fmul_rn(x, up), __fmul_rn(other, up), acc);
             if (!nan && !(acc & PC::FAST_BAD)) bad += w3 != (ref | (ref_o << 16));
             acc = 0;
+            const unsigned w5 = PC::enc1_fast(__fmul_rn(x, up), acc) & 0xFFFFu;                 // the one-code form
+            if (!nan && !(acc & PC::FAST_BAD)) bad += w5 != ref;
+            acc = 0;
             const unsigned w4 = PC::enc2_fast(__fmul_rn(x, up), __fmul_rn(x, up), acc);
             // (and it must claim validity on the whole regime of zeros: |2^7 x| < 1)
             if (!nan && (b & 0x7FFFFFFFu) < 0x3BFFF000u /* just below 2^-7 */) bad += (acc & PC::FAST_BAD) != 0 || w4 != (ref | (ref << 16));

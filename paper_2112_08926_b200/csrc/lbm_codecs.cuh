@@ -330,6 +330,11 @@ struct PairCodec<F_P16_0S> {
         const unsigned signs = __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x7632);
         return __byte_perm(ta, tb, 0x5410) | (signs & 0x80008000u);
     }
+    static __device__ __forceinline__ unsigned enc1_fast(float a, unsigned &acc) {          // one code (in the low 16 bits)
+        const unsigned ta = __float_as_uint(__fadd_rz(__fmaf_rz(fabsf(a), 4194304.0f, 0.5f), 8388608.0f)) ^ 0x4B000000u;
+        acc |= ta;
+        return ta | ((__float_as_uint(a) >> 16) & 0x8000u);
+    }
     static constexpr unsigned FAST_BAD = 0xFFFFC000u;       // acc & FAST_BAD != 0: outside enc2_fast's domain
 };
 

@@ -542,17 +542,41 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                         char *o = ostage + 2 * fp * ES;
                         full_mode = pull_cell<Q, F, ALT, 0>(stage + own_b, stage + left_b, stage + right_b, f, wd, warp_full);
                         collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f, p);
+                        if constexpr (PC::FAST) {                           // (the table-free encoder, as in the pair path below)
+                            unsigned acc = full_mode ? PC::FAST_BAD : 0u;
+                            if (!full_mode) {
 #pragma unroll
-                        for (int i = 0; i < Q; ++i) {
-                            if constexpr (ES == 4) *reinterpret_cast<float *>(o + i * SH::OPITCH) = f[i];
-                            else *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH) = (unsigned short)PC::enc1(f[i], tab);
+                                for (int i = 0; i < Q; ++i) *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH) = (unsigned short)PC::enc1_fast(f[i], acc);
+                            }
+                            if (acc & PC::FAST_BAD) {
+#pragma unroll
+                                for (int i = 0; i < Q; ++i) *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH) = (unsigned short)PC::enc1(f[i], tab);
+                            }
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < Q; ++i) {
+                                if constexpr (ES == 4) *reinterpret_cast<float *>(o + i * SH::OPITCH) = f[i];
+                                else *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH) = (unsigned short)PC::enc1(f[i], tab);
+                            }
                         }
                         full_mode |= pull_cell<Q, F, ALT, 1>(stage + own_b, stage + left_b, stage + right_b, f, wd, warp_full);
                         collide<COLL, Q, FORCE, SC, ES == 2 ? 1 : 2>(f, p);
+                        if constexpr (PC::FAST) {                           // (the table-free encoder, as in the pair path below)
+                            unsigned acc = full_mode ? PC::FAST_BAD : 0u;
+                            if (!full_mode) {
 #pragma unroll
-                        for (int i = 0; i < Q; ++i) {
-                            if constexpr (ES == 4) *reinterpret_cast<float *>(o + i * SH::OPITCH + 4) = f[i];
-                            else *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH + 2) = (unsigned short)PC::enc1(f[i], tab);
+                                for (int i = 0; i < Q; ++i) *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH + 2) = (unsigned short)PC::enc1_fast(f[i], acc);
+                            }
+                            if (acc & PC::FAST_BAD) {
+#pragma unroll
+                                for (int i = 0; i < Q; ++i) *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH + 2) = (unsigned short)PC::enc1(f[i], tab);
+                            }
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < Q; ++i) {
+                                if constexpr (ES == 4) *reinterpret_cast<float *>(o + i * SH::OPITCH + 4) = f[i];
+                                else *reinterpret_cast<unsigned short *>(o + i * SH::OPITCH + 2) = (unsigned short)PC::enc1(f[i], tab);
+                            }
                         }
                     }
                 } else if (fp < pairs) {
