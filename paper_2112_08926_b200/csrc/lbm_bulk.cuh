@@ -60,6 +60,9 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned byt
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive_n(unsigned bar, unsigned count) {          // `count` arrivals at once
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
 // the same with a suspend-time hint: a waiting thread sleeps until the phase completes (or the hint, in ns, runs out)
 // instead of coming back to poll -- polling warps take issue slots from the arithmetic warps
 __device__ __forceinline__ void mbar_wait_sleepy(unsigned bar, unsigned parity) {

@@ -85,6 +85,11 @@ struct StageShape {
     // 96-register posit kernels -- a thread finishes its first cell (pull, collide, encode, half-word stores) before it
     // pulls the second
     static constexpr bool SPLIT = Q == 27 || MANY;
+    // chunk ids a warp takes at a time.  The per-claim work (the counter, two barrier waits, the header, two arrivals, the
+    // list-pass test) is about 40 of the 120 non-arithmetic warp-instructions per chunk: against D2Q9's nine directions that
+    // is a tenth of the kernel, and its 2048-cell tiles have 32 chunks, so two at a time still leave 16 claims per tile.
+    // D3Q19 (16 chunks per tile, 14 warps) loses 5-10% on 256^3 boxes with two: one there.
+    static constexpr int CPC = (Q == 9 && ES == 2) ? 2 : 1;
     static constexpr int NCT = 32 * NCW, NT = NCT + 64;                                 // + the loader and the storer warp
     static constexpr int WLAG = 3;                          // the storer reports a tile written WLAG tiles later (the bulk-copy
                                                             // engine's write may take that long; waiting for it earlier stalls the storer)
@@ -511,10 +516,10 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
 #pragma unroll 1
     for (;;) {
         unsigned id = 0;
-        if (lane == 0) id = atomicAdd(counter, 1u);
+        if (lane == 0) id = atomicAdd(counter, (unsigned)SH::CPC);           // ids id .. id + CPC - 1, all of one tile (2^shift >= 8)
         id = __shfl_sync(0xffffffffu, id, 0);
         if (id >= n_ids) break;
-        const int k = (int)(id >> shift), c = (int)(id & ((1u << shift) - 1u));
+        const int k = (int)(id >> shift), c0 = (int)(id & ((1u << shift) - 1u));
         if (k < my_tiles) {
             const int si = k % S_IN, so = k % S_OUT;
             const char *stage = smem + si * SH::INB;
@@ -525,6 +530,8 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
             // arrival below must not count for the stage's previous use.)  Waiting here, not between the collision and
             // the stores, lets every result go to shared memory as soon as it exists.
             if (k >= S_OUT) mbar_wait(bar_out_empty + so * 8, (unsigned)(k / S_OUT - 1) & 1u);
+#pragma unroll 1
+            for (int c = c0; c < c0 + SH::CPC; ++c) {
             const int fp = 32 * c + lane;
             if (32 * c < pairs) {
                 // the pair's place in a direction's segment and in the row (only the row ends matter: x wraps)
@@ -610,11 +617,12 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                     }
                 }
             }
+            }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_in_empty + si * 8);              // once every chunk has: the input stage may be refilled
+            if (lane == 0) mbar_arrive_n(bar_in_empty + si * 8, SH::CPC);   // once every chunk id has: the input stage may be refilled
             fence_async_smem();                                             // this thread's writes -> visible to the bulk-copy engine
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_out_full + so * 8);
+            if (lane == 0) mbar_arrive_n(bar_out_full + so * 8, SH::CPC);
         }
         // The list pass.  The lists of LG consecutive tiles of this CTA (a group; the last one may be shorter) are walked
         // together, LAG tiles after the group's last tile was computed, when its bulk store is complete (`done`; stores
@@ -644,8 +652,10 @@ stream_collide_staged_kernel(const typename Elem<F>::T *__restrict__ A, typename
                     end[gi] = total;
                 }
                 if (total != 0) {
-                    const unsigned share = (((total + (1u << shift) - 1u) >> shift) + 31u) & ~31u;
-                    const unsigned a = (unsigned)c * share, b = min(total, a + share);
+                    // (one share per claim of CPC chunk ids: 2^shift / CPC shares)
+                    constexpr int CS = SH::CPC == 2 ? 1 : 0;
+                    const unsigned share = (((total + (1u << (shift - CS)) - 1u) >> (shift - CS)) + 31u) & ~31u;
+                    const unsigned a = (unsigned)(c0 >> CS) * share, b = min(total, a + share);
                     if (a < b) {
                         mbar_wait(bar_done + (jhi % SH::DONES) * 8, (unsigned)(jhi / SH::DONES) & 1u);
                         fence_async_global();
