@@ -139,7 +139,8 @@ int ensure_ddf(lbm *h) {
 
 // Kernel variant.  Automatic choice, from the sweeps recorded in DESIGN.md section 6:
 //   * FP64 arithmetic: one kernel, one cell per thread (lbm_fp64.cuh);
-//   * rows 16-cell aligned and >= 64 cells, box >= 2^20 cells, and either a 16-bit format or a box with flagged cells:
+//   * rows 16-cell aligned and >= 64 cells, box >= 2^20 cells (2^19 with flagged cells), and either a 16-bit format or a box
+//     with flagged cells:
 //     the warp-specialised staged kernel (lbm_stage.cuh) -- it lifts the 16-bit formats out of the issue bound and
 //     handles flagged cells in a compacted list pass instead of a divergent slow path;
 //   * FP32 storage without flagged cells: the per-thread kernel, which runs at the HBM roofline;
@@ -150,7 +151,9 @@ int pick_variant(const lbm *h) {
     int want = h->V_request;
     const bool staged_ok = h->nx % 16 == 0 && (long long)((h->nx + h->ops->staged_tile_cells() - 1) / h->ops->staged_tile_cells()) * h->ny * h->nz < 0x7FFFFFFFLL;
     if (want == LBM_VARIANT_STAGED && staged_ok) return LBM_VARIANT_STAGED;
-    if (want == 0 && staged_ok && (h->fmt != LBM_FP32 || h->has_walls) && h->nx >= 64 && h->N >= (1LL << 20)) return LBM_VARIANT_STAGED;
+    // (boxes with flagged cells: from 2^19 cells -- the per-thread kernel's wall path is 1.1-1.6 times slower there already)
+    if (want == 0 && staged_ok && (h->fmt != LBM_FP32 || h->has_walls) && h->nx >= 64 && h->N >= (h->has_walls ? (1LL << 19) : (1LL << 20)))
+        return LBM_VARIANT_STAGED;
     if (want != 1 && want != 2 && want != 4) want = (h->q == LBM_D2Q9 && h->fmt != LBM_FP32) ? 4 : 2;
     while (want > 1 && h->nx % want != 0) want >>= 1;
     return want;
