@@ -91,13 +91,17 @@ struct StageShape {
     // D3Q19 (16 chunks per tile, 14 warps) loses 5-10% on 256^3 boxes with two: one there.
     static constexpr int CPC = (Q == 9 && ES == 2) ? 2 : 1;
     static constexpr int NCT = 32 * NCW, NT = NCT + 64;                                 // + the loader and the storer warp
-    static constexpr int WLAG = 3;                          // the storer reports a tile written WLAG tiles later (the bulk-copy
-                                                            // engine's write may take that long; waiting for it earlier stalls the storer)
-    static constexpr int LAG = WLAG + 1;                    // the list pass of a tile runs at least LAG tiles later ...
-    // ... together with the lists of its group of LG consecutive tiles.  Measured (cavity 256^3): grouping gives the
-    // instruction-bound 16-bit kernels +2% (FP16S) to +34% (P16_1S) and costs the FP32 kernel, which waits for memory
-    // anyway, 8% -- FP32 keeps one list per pass
-    static constexpr int LG = ES == 4 ? 1 : 4;
+    // The storer reports tile k written WLAG tiles later, and the list pass of a tile runs LAG = WLAG + 1 tiles after it,
+    // together with the lists of its group of LG consecutive tiles.  Both are as SHORT as they can be: the list pass
+    // re-reads, sector by sector, values that the main pass streamed through L2 a moment ago, and the sooner it comes the
+    // more of them are still there -- cavity 256^3, WLAG = 3 -> 0: FP32 32.1 -> 35.5, FP16S 50.9 -> 54.9 GLUPs/s, although the
+    // storer now waits for each tile's writes before it sends the next.  Grouping fills the lanes of the warps that
+    // walk the lists (a cavity tile has a dozen listed cells): LG = 4 gives the instruction-bound formats +24% (FP16C) to
+    // +34% (P16_1S); the lighter kernels (FP32, FP16S, FP16), which feel the re-reads more, are best with 2 (FP16S 58.0
+    // against 54.8 with 4 and 52.7 with 1; FP32 37.4 against 35.5 with 1).
+    static constexpr int WLAG = 0;
+    static constexpr int LAG = WLAG + 1;
+    static constexpr int LG = (ES == 4 || F == F_FP16S || F == F_FP16) ? 2 : 4;
     static constexpr int ROWB = TC * ES + 2 * PAD;          // one direction of one input stage
     static constexpr int INB = in_bytes(TC);
     static constexpr int OPITCH = TC * ES;                  // one direction of one output stage
